@@ -1,0 +1,179 @@
+/*
+ * pce.h -- C ABI of the B200 polarizable-colloid electrostatics library
+ * (hot path of arxiv 2401.04865; citations are lines of the paper text,
+ * "PAPER.md:N", with the equation they fall in).
+ *
+ * What the library computes
+ * -------------------------
+ * N particles (surface beads of N_body rigid conductors, then ions) of one
+ * radius a in a triply periodic box.  The potential tensor (eq. 9)
+ *     M_ab = 1/(eps_f V) sum_{k != 0} j0(ka)^2 exp(i k.(x_a-x_b)) / k^2
+ * is applied by the spectral Ewald method of PAPER.md:167-268 (real-space sum
+ * eq. 20-21, Gaussian spreading eq. 25, FFT, scaling eq. 26, inverse FFT,
+ * Gaussian gather eq. 27), the induced bead charges follow from the
+ * saddle-point system eq. 13 solved by a Krylov iteration on
+ * the device, and energies / forces / torques from eqs. 14, 16-18
+ * (PAPER.md:137-163).
+ *
+ * Conventions
+ * -----------
+ *  - every entry point returns 0 (PCE_OK) or a negative pce_status; no
+ *    exception crosses the boundary; pce_last_error() gives the text.
+ *  - "device" pointers are CUDA device memory of fp64 unless stated, owned by
+ *    the CALLER (e.g. torch tensors), never retained past the call unless
+ *    stated; "host" pointers are ordinary host memory.  The context owns all
+ *    workspace (grids, cuFFT plans, cell lists, CSR near field, Krylov
+ *    vectors) and frees it in pce_destroy.
+ *  - all work is enqueued on the stream given to pce_create (a cudaStream_t
+ *    passed as void*; NULL = default stream).  Calls are asynchronous except
+ *    pce_solve (reads the residual) and pce_step_host.
+ *  - particle order (structure of Sigma, eq. 52): beads of
+ *    body 0, body 1, ... contiguous, then ions.  body_offset[N_body+1] (host,
+ *    int32) gives the bead ranges; N_bead = body_offset[N_body].
+ *  - SoA: x, y, z separate arrays.  Positions may lie outside [0,L); they
+ *    are wrapped internally.  Results come back in caller order.
+ *  - fp64 throughout.  There is no CPU fallback: without a CUDA device
+ *    pce_create fails with PCE_ECUDA.
+ */
+#ifndef PCE_H
+#define PCE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pce_ctx pce_ctx;
+
+typedef enum {
+    PCE_OK = 0,
+    PCE_EINVAL = -1,   /* bad parameter / shape / NULL pointer */
+    PCE_ENOMEM = -2,   /* device allocation failed */
+    PCE_ECUDA = -3,    /* CUDA runtime error (text in pce_last_error) */
+    PCE_ECUFFT = -4,   /* cuFFT plan / exec error */
+    PCE_ENOCONV = -5,  /* Krylov solve hit max_iter; outputs still written */
+    PCE_ESTATE = -6    /* call order violated (e.g. solve before set_system) */
+} pce_status;
+
+/* Parameters of the spectral Ewald sum and of the solver.
+ * eta is NOT a free input: eta = h^2 xi^2 P / pi (eq. 31,
+ * PAPER.md:250), per dimension for a rectangular box. */
+typedef struct {
+    double L[3];        /* box edge lengths */
+    int    Ng[3];       /* FFT grid nodes per dimension; each >= P */
+    double xi;          /* Ewald splitting parameter, h(k)=exp(-k^2/4xi^2) */
+    double rc;          /* real-space cut-off r_c (eq. 23); may exceed L/2 */
+    int    P;           /* support grid points per dimension, even, 4..32 (eq. 29) */
+    double a;           /* bead = ion radius: the shell regularization width (eq. 9-10) */
+    double eps_f;       /* fluid permittivity (1 in the paper's units) */
+    double tol_solver;  /* relative residual at which the Krylov solve stops */
+    int    max_iter;    /* iteration cap of the Krylov solve */
+    int    flags;       /* reserved, 0 */
+} pce_params;
+
+typedef struct {
+    int    iters;       /* Krylov iterations taken */
+    int    matvecs;     /* applications of M inside pce_solve (bead-only + full) */
+    double rel_resid;   /* final |P(b - M q)| / (|P r.E0|^2 + |P psi0|^2)^(1/2) */
+    int    converged;   /* 1 if rel_resid <= tol_solver */
+} pce_solve_info;
+
+/* Per-pass device times (ms, CUDA events on the context's stream) summed over
+ * the passes of the LAST pce_matvec / pce_evaluate / pce_solve / pce_forces
+ * call that ran with timing enabled (pce_set_timing). */
+typedef struct {
+    double cells, real, spread, fft, scale, ifft, gather, krylov, other, total;
+    int    n_matvec_bead, n_eval_full;
+} pce_timings;
+
+/* Derived quantities, for reports and tests. */
+typedef struct {
+    double eta[3], h[3];
+    int    ncell[3];        /* real-space linked cells per dimension */
+    int    image_range[3];  /* >0: periodic images summed explicitly in that dimension */
+    long long nnz_near;     /* entries of the cached bead-bead near field */
+    int    N, N_bead, N_body;
+    long long bytes_workspace;
+} pce_info;
+
+/* Ewald parameters from a target tolerance (pure host arithmetic):
+ * s^2 = -ln tol; k_c = pi (Ng-1)/L; xi = k_c/(2s) (eq. 28);
+ * r_c = s/xi + 2a (eq. 23; the +2a because eq. 20 decays like
+ * erfc((r-2a) xi) for shells, reading A14); P even with
+ * exp(-pi P/2) a factor ~500 below tol (eq. 32).  P_override > 0 fixes P.
+ * Fills L, Ng, xi, rc, P, a, eps_f=1, tol_solver=1e-12, max_iter=500. */
+int pce_suggest_params(const double L[3], const int Ng[3], double a, double tol,
+                       int P_override, pce_params* out);
+
+/* Create a context on the current CUDA device.  `stream` is a cudaStream_t. */
+int pce_create(const pce_params* p, void* stream, pce_ctx** out);
+int pce_destroy(pce_ctx* ctx);
+const char* pce_last_error(const pce_ctx* ctx); /* ctx may be NULL: last create error */
+
+/* Declare the particle system and its positions (device x,y,z of length N).
+ * body_offset: host int32[N_body+1], body_offset[0]=0, non-decreasing,
+ * body_offset[N_body] = N_bead <= N.  Builds the linked cells,
+ * body centres X_i (mean of the body's beads unwrapped about its first bead,
+ * "centre of mass" PAPER.md:115) and r_ij = x_ij - X_i (eq. 12), and the
+ * cached bead-bead real-space near field. */
+int pce_set_system(pce_ctx* ctx, int N, int N_body, const int* body_offset,
+                   const double* x, const double* y, const double* z);
+/* New positions for the same system (e.g. next time step). */
+int pce_set_positions(pce_ctx* ctx, const double* x, const double* y, const double* z);
+
+/* psi = M_bb q over the N_bead conductor beads only (the solver's matvec;
+ * eq. 8, restricted to bead sources and bead targets).
+ * q, psi: device, length N_bead, caller order. */
+int pce_matvec(pce_ctx* ctx, const double* q, double* psi);
+
+/* Potentials psi_a - psi_0(x_a) = sum_b M_ab q_b (eq. 8 / eq. 19) and fields
+ * E_a = -grad_a sum_b M_ab q_b (excludes E0; the b = a term has no gradient)
+ * at all N particles from all N charges.  q, psi, Ex, Ey, Ez: device, length
+ * N.  The three field pointers may all be NULL (potential only). */
+int pce_evaluate(pce_ctx* ctx, const double* q, double* psi,
+                 double* Ex, double* Ey, double* Ez);
+
+/* Induced charges: eq. 13 with the ions as one-bead bodies of
+ * fixed charge:  sum_j q_ij = Q_i  and
+ * psi_ij - psi_0,ij = Phi_i + r_ij.E0,  Phi_i = Psi_i - Psi_0,i  (eq. 12).
+ *  Q_body : device [N_body]; q_ion : device [N - N_bead] (may be NULL if no ions)
+ *  E0     : host [3]
+ *  q      : device [N]; out: bead charges then the ion charges.  If
+ *           warm_start != 0 its bead part is read as the initial guess.
+ *  Phi_body : device [N_body] out.
+ * Method: conjugate gradients on the per-body-mean-projected SPD system,
+ * whole iteration on the device.  Returns PCE_ENOCONV if max_iter was hit. */
+int pce_solve(pce_ctx* ctx, const double* Q_body, const double* q_ion, const double E0[3],
+              int warm_start, double* q, double* Phi_body, pce_solve_info* info);
+
+/* Forces, torques, dipoles, energies for given charges q (device [N]):
+ *  f_a = q_a (E0 + E_a)                               eq. 17
+ *  F_i = sum_j f_ij,  T_i = sum_j r_ij x f_ij          eq. 18
+ *  S_i = sum_j r_ij q_ij                               eq. 14
+ *  U_i = (Q_i Psi_i - S_i.E0)/2, Psi_i = <psi_ij - r_ij.E0>_i - X_i.E0   eq. 16
+ * Outputs (device; any may be NULL): fx,fy,fz [N]; F,T,S [3*N_body] as
+ * (x[N_body], y[N_body], z[N_body]); U_body [N_body + N_ion] (ions:
+ * q (psi - x.E0)/2); U_tot [3] = (U_eq16, W, U_MM) with U_MM = q.M.q/2 and
+ * W = U_MM - sum_a q_a x_a.E0 (reading A8); psi [N] potentials. */
+int pce_forces(pce_ctx* ctx, const double* q, const double E0[3],
+               double* fx, double* fy, double* fz,
+               double* F, double* T, double* S, double* U_body, double* U_tot, double* psi);
+
+/* One whole pass of the hot path from HOST buffers (what bench.py's "e2e"
+ * times): copy positions and charges to the device, rebuild cells, solve
+ * eq. 13, evaluate forces, copy results back.  All pointers host; x,y,z [N];
+ * outputs as in pce_solve / pce_forces (any output may be NULL). */
+int pce_step_host(pce_ctx* ctx, const double* x, const double* y, const double* z,
+                  const double* Q_body, const double* q_ion, const double E0[3],
+                  double* q, double* Phi_body, double* fx, double* fy, double* fz,
+                  double* F, double* T, double* S, double* U_tot, pce_solve_info* info);
+
+int pce_set_timing(pce_ctx* ctx, int enabled);          /* per-pass CUDA events on/off (default off) */
+int pce_get_timings(const pce_ctx* ctx, pce_timings* t);
+int pce_get_info(const pce_ctx* ctx, pce_info* info);
+/* number of kernels of this library (cuFFT's own excluded) launched since create */
+long long pce_launch_count(const pce_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCE_H */

@@ -1,0 +1,477 @@
+// pce_api.cu -- the C ABI of include/pce.h: context, parameter derivation
+// (eqs. 23, 28, 31, 32), orchestration of the spectral Ewald passes
+// (steps 1-6) and per-pass timing.
+#include "pce_internal.h"
+
+#include <cmath>
+
+static std::string g_create_err;
+
+// ---------------------------------------------------------------- parameters
+extern "C" int pce_suggest_params(const double L[3], const int Ng[3], double a, double tol, int P_override, pce_params* out)
+{
+    if (!L || !Ng || !out || !(tol > 0.0 && tol < 1.0) || !(a > 0.0)) return PCE_EINVAL;
+    for (int d = 0; d < 3; ++d)
+        if (!(L[d] > 0.0) || Ng[d] < 4) return PCE_EINVAL;
+    const double s = std::sqrt(-std::log(tol));
+    double kc = 1e300;
+    for (int d = 0; d < 3; ++d) kc = std::fmin(kc, PCE_PI * (Ng[d] - 1) / L[d]);  // N_g = 1 + L k_c / pi
+    const double xi = kc / (2.0 * s);                                            // exp(-k_c^2/4xi^2) = tol (eq. 28)
+    const double rc = s / xi + 2.0 * a;                                          // eq. 23, shells: erfc((r-2a) xi)
+    int P = P_override;
+    if (P <= 0) {
+        const double p0 = (2.0 / PCE_PI) * (-std::log(tol)) + 4.0;               // exp(-pi P/2) <~ tol e^{-2 pi} (eq. 32)
+        P = 2 * (int)std::ceil(p0 / 2.0);
+    }
+    if (P < 4) P = 4;
+    if (P > 32) P = 32;
+    for (int d = 0; d < 3; ++d)
+        if (P > Ng[d]) P = Ng[d] & ~1;
+    std::memset(out, 0, sizeof(*out));
+    for (int d = 0; d < 3; ++d) { out->L[d] = L[d]; out->Ng[d] = Ng[d]; }
+    out->xi = xi; out->rc = rc; out->P = P; out->a = a; out->eps_f = 1.0;
+    out->tol_solver = 1e-12; out->max_iter = 500; out->flags = 0;
+    return PCE_OK;
+}
+
+// ---------------------------------------------------------------- timing
+static void timing_begin(pce_ctx* c)
+{
+    std::memset(&c->tm, 0, sizeof(c->tm));
+    c->recs.clear();
+    c->ev_used = 0;
+}
+
+static void timing_end(pce_ctx* c)
+{
+    if (!c->timing) return;
+    cudaStreamSynchronize(c->st);
+    double* slot[PASS_COUNT] = {&c->tm.cells, &c->tm.real, &c->tm.spread, &c->tm.fft, &c->tm.scale,
+                                &c->tm.ifft,  &c->tm.gather, &c->tm.krylov, &c->tm.other};
+    for (auto& r : c->recs) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, r.a, r.b);
+        *slot[r.pass] += ms;
+        c->tm.total += ms;
+    }
+    c->recs.clear();
+    c->ev_used = 0;
+}
+
+// ---------------------------------------------------------------- create / destroy
+static void free_system(pce_ctx* c)
+{
+    cudaFree(c->x); cudaFree(c->y); cudaFree(c->z); cudaFree(c->body_off); cudaFree(c->body_of);
+    cudaFree(c->rx); cudaFree(c->ry); cudaFree(c->rz); cudaFree(c->X); cudaFree(c->Y); cudaFree(c->Z);
+    bins_free(c->all); bins_free(c->bead);
+    cudaFree(c->csr_ptr); cudaFree(c->csr_col); cudaFree(c->csr_val);
+    cudaFree(c->w_real); cudaFree(c->w_wave); cudaFree(c->w_ex); cudaFree(c->w_ey); cudaFree(c->w_ez);
+    cudaFree(c->w_kx); cudaFree(c->w_ky); cudaFree(c->w_kz);
+    cudaFree(c->cg_g); cudaFree(c->cg_p); cudaFree(c->cg_t); cudaFree(c->cg_ap); cudaFree(c->cg_psi); cudaFree(c->cg_rhs);
+    cudaFree(c->ev_psi); cudaFree(c->ev_ex); cudaFree(c->ev_ey); cudaFree(c->ev_ez); cudaFree(c->cg_scal);
+    cudaFree(c->hs_dev);
+    c->x = c->y = c->z = nullptr; c->body_off = c->body_of = nullptr;
+    c->rx = c->ry = c->rz = c->X = c->Y = c->Z = nullptr;
+    c->csr_ptr = c->csr_col = nullptr; c->csr_val = nullptr; c->nnz = c->nnz_cap = 0;
+    c->w_real = c->w_wave = c->w_ex = c->w_ey = c->w_ez = c->w_kx = c->w_ky = c->w_kz = nullptr;
+    c->cg_g = c->cg_p = c->cg_t = c->cg_ap = c->cg_psi = c->cg_rhs = nullptr;
+    c->ev_psi = c->ev_ex = c->ev_ey = c->ev_ez = c->cg_scal = nullptr;
+    c->hs_dev = nullptr; c->hs_dev_n = 0;
+    c->have_system = false;
+}
+
+extern "C" int pce_destroy(pce_ctx* c)
+{
+    if (!c) return PCE_EINVAL;
+    cudaStreamSynchronize(c->st);
+    free_system(c);
+    if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->scan_tmp);
+    for (auto e : c->ev_pool) cudaEventDestroy(e);
+    delete c;
+    return PCE_OK;
+}
+
+extern "C" const char* pce_last_error(const pce_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+static int create_impl(pce_ctx* c)
+{
+    const pce_params& p = c->p;
+    c->V = p.L[0] * p.L[1] * p.L[2];
+    WaveConst& w = c->wk;
+    double cn2 = 1.0, h3 = 1.0, ntot = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        c->h[d] = p.L[d] / p.Ng[d];
+        c->eta[d] = c->h[d] * c->h[d] * p.xi * p.xi * p.P / PCE_PI;  // eq. 31
+        w.Ng[d] = p.Ng[d]; w.L[d] = p.L[d]; w.h[d] = c->h[d]; w.inv_h[d] = 1.0 / c->h[d];
+        w.kfac[d] = 2.0 * PCE_PI / p.L[d];
+        w.gexp[d] = (1.0 - c->eta[d]) / (4.0 * p.xi * p.xi);
+        w.grad_fac[d] = 4.0 * PCE_PI / (p.P * c->h[d]);
+        cn2 *= 2.0 / (p.P * c->h[d] * c->h[d]);
+        h3 *= c->h[d];
+        ntot *= p.Ng[d];
+    }
+    w.Nxh = p.Ng[0] / 2 + 1;
+    w.P = p.P;
+    w.aw = 2.0 * PCE_PI / p.P;
+    w.a = p.a;
+    w.scale_norm = cn2 * h3 / (p.eps_f * ntot);
+    RealConst& r = c->rk;
+    r.a = p.a; r.xi = p.xi; r.two_a = 2.0 * p.a; r.inv_eps = 1.0 / p.eps_f;
+    r.c64 = 1.0 / (64.0 * PCE_PI * p.a * p.a * p.xi * p.xi);
+    r.rc2 = p.rc * p.rc;
+    const double pi32 = PCE_PI * std::sqrt(PCE_PI);
+    const double e4 = std::exp(-4.0 * p.a * p.a * p.xi * p.xi);
+    r.R0 = (1.0 - e4) / (8.0 * pi32 * p.a * p.a * p.xi) + std::erfc(2.0 * p.a * p.xi) / (4.0 * PCE_PI * p.a);  // eq. 21
+    r.two_xi_sqrtpi = 2.0 * p.xi / std::sqrt(PCE_PI);
+    r.t_lin = 1.0 / (16.0 * PCE_PI * p.a * p.a);
+    r.t_quad = p.xi * (1.0 - e4) / (24.0 * pi32 * p.a * p.a);
+    r.r_small = 1e-3 * p.a;
+    c->kconst = 1.0 / (4.0 * p.xi * p.xi * c->V * p.eps_f);  // k = 0 removal (reading A1)
+
+    const size_t ng = (size_t)p.Ng[0] * p.Ng[1] * p.Ng[2];
+    const size_t nk = (size_t)w.Nxh * p.Ng[1] * p.Ng[2];
+    if (cudaMalloc(&c->grid, ng * sizeof(double)) != cudaSuccess || cudaMalloc(&c->gridk, nk * sizeof(cufftDoubleComplex)) != cudaSuccess) {
+        c->err = "out of device memory for the FFT grids";
+        return PCE_ENOMEM;
+    }
+    c->bytes += (long long)(ng * 8 + nk * 16);
+    PCE_CUDA(c, cudaMalloc(&c->scal, 64 * sizeof(double)));
+    // cuFFT plans sharing one work area
+    size_t wsF = 0, wsB = 0;
+    if (cufftCreate(&c->planF) != CUFFT_SUCCESS || cufftCreate(&c->planB) != CUFFT_SUCCESS) { c->err = "cufftCreate failed"; return PCE_ECUFFT; }
+    c->have_plans = true;
+    cufftSetAutoAllocation(c->planF, 0);
+    cufftSetAutoAllocation(c->planB, 0);
+    if (cufftMakePlan3d(c->planF, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_D2Z, &wsF) != CUFFT_SUCCESS ||
+        cufftMakePlan3d(c->planB, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_Z2D, &wsB) != CUFFT_SUCCESS) {
+        c->err = "cuFFT cannot plan this grid";
+        return PCE_ECUFFT;
+    }
+    const size_t ws = wsF > wsB ? wsF : wsB;
+    if (ws > 0) {
+        if (cudaMalloc(&c->fft_work, ws) != cudaSuccess) { c->err = "out of device memory for the cuFFT work area"; return PCE_ENOMEM; }
+        c->bytes += (long long)ws;
+    }
+    cufftSetWorkArea(c->planF, c->fft_work);
+    cufftSetWorkArea(c->planB, c->fft_work);
+    cufftSetStream(c->planF, c->st);
+    cufftSetStream(c->planB, c->st);
+    return PCE_OK;
+}
+
+extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
+{
+    if (!p || !out) { g_create_err = "NULL argument"; return PCE_EINVAL; }
+    *out = nullptr;
+    bool ok = p->xi > 0 && p->rc > 0 && p->a > 0 && p->eps_f > 0 && p->P >= 4 && p->P <= 32 && (p->P % 2 == 0) && p->max_iter > 0 &&
+              p->tol_solver > 0;
+    for (int d = 0; d < 3 && ok; ++d) ok = p->L[d] > 0 && p->Ng[d] >= p->P && p->Ng[d] >= 4;
+    if (!ok) { g_create_err = "invalid pce_params (need xi,rc,a,eps_f>0; P even in 4..32; Ng>=P; max_iter>0)"; return PCE_EINVAL; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        g_create_err = "no CUDA device: this library has no CPU fallback";
+        return PCE_ECUDA;
+    }
+    pce_ctx* c = new pce_ctx();
+    c->p = *p;
+    c->st = (cudaStream_t)stream;
+    std::memset(&c->tm, 0, sizeof(c->tm));
+    int rc = create_impl(c);
+    if (rc != PCE_OK) {
+        g_create_err = c->err;
+        pce_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return PCE_OK;
+}
+
+// ---------------------------------------------------------------- system / positions
+static void cell_layout(const pce_params& p, int nc[3], int range[3])
+{
+    for (int d = 0; d < 3; ++d) {
+        int n = (int)std::floor(p.L[d] / p.rc);
+        if (n > 256) n = 256;
+        if (n >= 3) { nc[d] = n; range[d] = 1; }
+        else { nc[d] = 1; range[d] = (int)std::ceil(p.rc / p.L[d]); }  // explicit periodic images (reading A10)
+    }
+}
+
+#define ALLOC_D(ptr, n)                                                                                     \
+    do {                                                                                                    \
+        size_t n__ = (size_t)((n) > 0 ? (n) : 1);                                                           \
+        if (cudaMalloc(&(ptr), n__ * sizeof(double)) != cudaSuccess) { c->err = "out of device memory"; return PCE_ENOMEM; } \
+        c->bytes += (long long)(n__ * 8);                                                                   \
+    } while (0)
+
+static int positions_impl(pce_ctx* c, const double* x, const double* y, const double* z)
+{
+    int rc;
+    {
+        PassTimer t(c, PASS_CELLS);
+        if ((rc = wrap_positions(c, c->N, x, y, z, c->x, c->y, c->z))) return rc;
+        if ((rc = bins_build(c, c->all, c->x, c->y, c->z))) return rc;
+        if ((rc = bins_build(c, c->bead, c->x, c->y, c->z))) return rc;  // beads are the first Nbead particles
+        if ((rc = bodies_setup(c))) return rc;
+    }
+    if ((rc = real_csr_build(c, c->bead))) return rc;
+    return PCE_OK;
+}
+
+extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_offset, const double* x, const double* y, const double* z)
+{
+    if (!c) return PCE_EINVAL;
+    if (N <= 0 || N_body < 0 || !x || !y || !z || (N_body > 0 && !body_offset)) { c->err = "pce_set_system: bad arguments"; return PCE_EINVAL; }
+    std::vector<int> off(N_body + 1, 0);
+    for (int i = 0; i <= N_body && N_body > 0; ++i) off[i] = body_offset[i];
+    if (off[0] != 0) { c->err = "body_offset[0] must be 0"; return PCE_EINVAL; }
+    for (int i = 0; i < N_body; ++i)
+        if (off[i + 1] < off[i]) { c->err = "body_offset must be non-decreasing"; return PCE_EINVAL; }
+    if (off[N_body] > N) { c->err = "body_offset[N_body] exceeds N"; return PCE_EINVAL; }
+    timing_begin(c);
+    cudaStreamSynchronize(c->st);
+    free_system(c);
+    c->N = N; c->Nbody = N_body; c->Nbead = off[N_body]; c->Nion = N - c->Nbead;
+    c->body_off_h = off;
+    const int nb1 = N_body + 1;
+    ALLOC_D(c->x, N); ALLOC_D(c->y, N); ALLOC_D(c->z, N);
+    ALLOC_D(c->rx, c->Nbead); ALLOC_D(c->ry, c->Nbead); ALLOC_D(c->rz, c->Nbead);
+    ALLOC_D(c->X, N_body); ALLOC_D(c->Y, N_body); ALLOC_D(c->Z, N_body);
+    PCE_CUDA(c, cudaMalloc(&c->body_off, (size_t)nb1 * sizeof(int)));
+    PCE_CUDA(c, cudaMalloc(&c->body_of, (size_t)(c->Nbead > 0 ? c->Nbead : 1) * sizeof(int)));
+    PCE_CUDA(c, cudaMemcpyAsync(c->body_off, off.data(), (size_t)nb1 * sizeof(int), cudaMemcpyHostToDevice, c->st));
+    {
+        std::vector<int> bo((size_t)(c->Nbead > 0 ? c->Nbead : 1), 0);
+        for (int b = 0; b < N_body; ++b)
+            for (int j = off[b]; j < off[b + 1]; ++j) bo[j] = b;
+        PCE_CUDA(c, cudaMemcpyAsync(c->body_of, bo.data(), bo.size() * sizeof(int), cudaMemcpyHostToDevice, c->st));
+        PCE_CUDA(c, cudaStreamSynchronize(c->st));
+    }
+    int nc[3], range[3], rc;
+    cell_layout(c->p, nc, range);
+    if ((rc = bins_alloc(c, c->all, N, nc, range))) return rc;
+    if ((rc = bins_alloc(c, c->bead, c->Nbead, nc, range))) return rc;
+    PCE_CUDA(c, cudaMalloc(&c->csr_ptr, ((size_t)c->Nbead + 2) * sizeof(int)));
+    ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
+    ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
+    ALLOC_D(c->cg_g, c->Nbead); ALLOC_D(c->cg_p, c->Nbead); ALLOC_D(c->cg_t, c->Nbead); ALLOC_D(c->cg_ap, c->Nbead);
+    ALLOC_D(c->cg_psi, c->Nbead); ALLOC_D(c->cg_rhs, c->Nbead);
+    ALLOC_D(c->ev_psi, N); ALLOC_D(c->ev_ex, N); ALLOC_D(c->ev_ey, N); ALLOC_D(c->ev_ez, N);
+    ALLOC_D(c->cg_scal, 2 * (c->p.max_iter + 2) + 2 + 2 * N_body + 16);
+    c->have_system = true;
+    rc = positions_impl(c, x, y, z);
+    timing_end(c);
+    return rc;
+}
+
+extern "C" int pce_set_positions(pce_ctx* c, const double* x, const double* y, const double* z)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_set_positions before pce_set_system"; return PCE_ESTATE; }
+    if (!x || !y || !z) { c->err = "NULL positions"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = positions_impl(c, x, y, z);
+    timing_end(c);
+    return rc;
+}
+
+// ---------------------------------------------------------------- the operator
+__global__ void k_sum1(const double* __restrict__ in, int n, double* __restrict__ out)
+{
+    __shared__ double sh[32];
+    double v = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) v += in[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += sh[i];
+        out[0] = s;
+    }
+}
+
+// psi[perm[i]] = real + wave - (sum q)/(4 xi^2 V eps); fields likewise (no constant)
+__global__ void k_finalize(int n, const int* __restrict__ perm, const double* __restrict__ re, const double* __restrict__ wa,
+                           const double* __restrict__ qsum, double kconst, double* __restrict__ psi, int field,
+                           const double* __restrict__ rx, const double* __restrict__ ry, const double* __restrict__ rz,
+                           const double* __restrict__ kx, const double* __restrict__ ky, const double* __restrict__ kz,
+                           double* __restrict__ ex, double* __restrict__ ey, double* __restrict__ ez)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int j = perm[i];
+    psi[j] = re[i] + wa[i] - kconst * qsum[0];
+    if (field) { ex[j] = rx[i] + kx[i]; ey[j] = ry[i] + ky[i]; ez[j] = rz[i] + kz[i]; }
+}
+
+static int apply_operator(pce_ctx* c, Bins& b, bool use_csr, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
+{
+    const bool field = (Ex != nullptr);
+    const int n = b.n;
+    int rc;
+    {
+        PassTimer t(c, PASS_OTHER);
+        if ((rc = gather_by_perm(c, n, b.perm, q, b.qs))) return rc;
+        k_sum1<<<1, 1024, 0, c->st>>>(q, n, c->scal);
+        c->launches++;
+    }
+    if (use_csr) rc = real_csr_spmv(c, b, c->w_real);                                   // step 1 (cached), eq. 20-21
+    else rc = real_direct(c, b, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);           // step 1, eq. 20-21
+    if (rc) return rc;
+    if ((rc = wave_spread(c, b))) return rc;                                            // step 2, eq. 25
+    if ((rc = wave_fft_scale_ifft(c))) return rc;                                       // steps 3-5, eq. 26
+    if ((rc = wave_gather(c, b, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    {
+        PassTimer t(c, PASS_OTHER);
+        k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0, c->w_ex,
+                                                   c->w_ey, c->w_ez, c->w_kx, c->w_ky, c->w_kz, Ex, Ey, Ez);
+        c->launches++;
+    }
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+int op_matvec_bead(pce_ctx* c, const double* q, double* psi)
+{
+    c->tm.n_matvec_bead++;
+    return apply_operator(c, c->bead, true, q, psi, nullptr, nullptr, nullptr);
+}
+
+int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
+{
+    c->tm.n_eval_full++;
+    return apply_operator(c, c->all, false, q, psi, Ex, Ey, Ez);
+}
+
+extern "C" int pce_matvec(pce_ctx* c, const double* q, double* psi)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_matvec before pce_set_system"; return PCE_ESTATE; }
+    if (!q || !psi) { c->err = "NULL argument"; return PCE_EINVAL; }
+    if (c->Nbead == 0) return PCE_OK;
+    timing_begin(c);
+    int rc = op_matvec_bead(c, q, psi);
+    timing_end(c);
+    return rc;
+}
+
+extern "C" int pce_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_evaluate before pce_set_system"; return PCE_ESTATE; }
+    const int nf = (Ex != nullptr) + (Ey != nullptr) + (Ez != nullptr);
+    if (!q || !psi || (nf != 0 && nf != 3)) { c->err = "NULL argument (field pointers: all or none)"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = op_evaluate(c, q, psi, Ex, Ey, Ez);
+    timing_end(c);
+    return rc;
+}
+
+extern "C" int pce_solve(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm_start, double* q,
+                         double* Phi_body, pce_solve_info* info)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_solve before pce_set_system"; return PCE_ESTATE; }
+    if (!E0 || !q || (c->Nbody > 0 && (!Q_body || !Phi_body))) { c->err = "NULL argument"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = solve_cg(c, Q_body, q_ion, E0, warm_start, q, Phi_body, info);
+    timing_end(c);
+    return rc;
+}
+
+extern "C" int pce_forces(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
+                          double* S, double* U_body, double* U_tot, double* psi)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_forces before pce_set_system"; return PCE_ESTATE; }
+    if (!q || !E0) { c->err = "NULL argument"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = forces_all(c, q, E0, fx, fy, fz, F, T, S, U_body, U_tot, psi);
+    timing_end(c);
+    return rc;
+}
+
+// ---------------------------------------------------------------- host-buffer pass (bench "e2e")
+extern "C" int pce_step_host(pce_ctx* c, const double* x, const double* y, const double* z, const double* Q_body, const double* q_ion,
+                             const double E0[3], double* q, double* Phi_body, double* fx, double* fy, double* fz, double* F, double* T,
+                             double* S, double* U_tot, pce_solve_info* info)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_step_host before pce_set_system"; return PCE_ESTATE; }
+    if (!x || !y || !z || !E0 || (c->Nbody > 0 && !Q_body) || (c->Nion > 0 && !q_ion)) { c->err = "NULL argument"; return PCE_EINVAL; }
+    const size_t N = c->N, nb = c->Nbody, ni = c->Nion;
+    const size_t need = 3 * N + nb + ni + N + nb + 3 * N + 9 * nb + 3 + 8;
+    if (need > c->hs_dev_n) {
+        cudaFree(c->hs_dev);
+        c->hs_dev = nullptr;
+        if (cudaMalloc(&c->hs_dev, need * sizeof(double)) != cudaSuccess) { c->err = "out of device memory (host staging)"; c->hs_dev_n = 0; return PCE_ENOMEM; }
+        c->hs_dev_n = need;
+    }
+    double* d = c->hs_dev;
+    double *dx = d, *dy = d + N, *dz = d + 2 * N, *dQ = d + 3 * N, *dqi = dQ + nb, *dq = dqi + ni, *dPhi = dq + N;
+    double *dfx = dPhi + nb, *dfy = dfx + N, *dfz = dfy + N, *dF = dfz + N, *dT = dF + 3 * nb, *dS = dT + 3 * nb, *dU = dS + 3 * nb;
+    timing_begin(c);
+    const bool tsave = c->timing;
+    PCE_CUDA(c, cudaMemcpyAsync(dx, x, N * 8, cudaMemcpyHostToDevice, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(dy, y, N * 8, cudaMemcpyHostToDevice, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(dz, z, N * 8, cudaMemcpyHostToDevice, c->st));
+    if (nb) PCE_CUDA(c, cudaMemcpyAsync(dQ, Q_body, nb * 8, cudaMemcpyHostToDevice, c->st));
+    if (ni) PCE_CUDA(c, cudaMemcpyAsync(dqi, q_ion, ni * 8, cudaMemcpyHostToDevice, c->st));
+    int rc = positions_impl(c, dx, dy, dz);
+    int rc_solve = PCE_OK;
+    if (!rc) {
+        rc_solve = solve_cg(c, dQ, dqi, E0, 0, dq, dPhi, info);
+        if (rc_solve != PCE_OK && rc_solve != PCE_ENOCONV) rc = rc_solve;
+    }
+    if (!rc) rc = forces_all(c, dq, E0, dfx, dfy, dfz, dF, dT, dS, nullptr, dU, nullptr);
+    if (!rc) {
+        if (q) PCE_CUDA(c, cudaMemcpyAsync(q, dq, N * 8, cudaMemcpyDeviceToHost, c->st));
+        if (Phi_body && nb) PCE_CUDA(c, cudaMemcpyAsync(Phi_body, dPhi, nb * 8, cudaMemcpyDeviceToHost, c->st));
+        if (fx) PCE_CUDA(c, cudaMemcpyAsync(fx, dfx, N * 8, cudaMemcpyDeviceToHost, c->st));
+        if (fy) PCE_CUDA(c, cudaMemcpyAsync(fy, dfy, N * 8, cudaMemcpyDeviceToHost, c->st));
+        if (fz) PCE_CUDA(c, cudaMemcpyAsync(fz, dfz, N * 8, cudaMemcpyDeviceToHost, c->st));
+        if (F && nb) PCE_CUDA(c, cudaMemcpyAsync(F, dF, 3 * nb * 8, cudaMemcpyDeviceToHost, c->st));
+        if (T && nb) PCE_CUDA(c, cudaMemcpyAsync(T, dT, 3 * nb * 8, cudaMemcpyDeviceToHost, c->st));
+        if (S && nb) PCE_CUDA(c, cudaMemcpyAsync(S, dS, 3 * nb * 8, cudaMemcpyDeviceToHost, c->st));
+        if (U_tot) PCE_CUDA(c, cudaMemcpyAsync(U_tot, dU, 3 * 8, cudaMemcpyDeviceToHost, c->st));
+        PCE_CUDA(c, cudaStreamSynchronize(c->st));
+    }
+    (void)tsave;
+    timing_end(c);
+    return rc ? rc : rc_solve;
+}
+
+// ---------------------------------------------------------------- reports
+extern "C" int pce_set_timing(pce_ctx* c, int enabled)
+{
+    if (!c) return PCE_EINVAL;
+    c->timing = enabled != 0;
+    return PCE_OK;
+}
+
+extern "C" int pce_get_timings(const pce_ctx* c, pce_timings* t)
+{
+    if (!c || !t) return PCE_EINVAL;
+    *t = c->tm;
+    return PCE_OK;
+}
+
+extern "C" int pce_get_info(const pce_ctx* c, pce_info* info)
+{
+    if (!c || !info) return PCE_EINVAL;
+    std::memset(info, 0, sizeof(*info));
+    for (int d = 0; d < 3; ++d) {
+        info->eta[d] = c->eta[d]; info->h[d] = c->h[d];
+        info->ncell[d] = c->all.nc[d];
+        info->image_range[d] = (c->all.nc[d] == 1) ? c->all.range[d] : 0;
+    }
+    info->nnz_near = c->nnz;
+    info->N = c->N; info->N_bead = c->Nbead; info->N_body = c->Nbody;
+    info->bytes_workspace = c->bytes;
+    return PCE_OK;
+}
+
+extern "C" long long pce_launch_count(const pce_ctx* c) { return c ? c->launches : 0; }

@@ -1,0 +1,180 @@
+// pce_internal.h -- shared declarations of the CUDA implementation (not part of the ABI).
+// Product code: never includes or links anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "pce.h"
+
+#define PCE_PI 3.14159265358979323846
+
+// ---------------------------------------------------------------- binning
+// A counting-sort binning of a particle subset into a Cartesian cell grid
+// (linked-cell neighbour search).  In a dimension with fewer
+// than 3 cells of size >= r_c the grid collapses to ONE cell and periodic
+// images -range..range are summed explicitly (covers r_c > L/2).
+struct Bins {
+    int n = 0;          // particles in the subset
+    int nc[3] = {1, 1, 1};
+    int ncell = 1;
+    int range[3] = {1, 1, 1};  // stencil half width: 1 (cells) or image count
+    double L[3];
+    int* cell_of = nullptr;     // [n]
+    int* cell_start = nullptr;  // [ncell+1]
+    int* cell_fill = nullptr;   // [ncell+1] scratch
+    int* perm = nullptr;        // [n] sorted slot -> index in the subset
+    int* perm_tmp = nullptr;    // [n]
+    double *xs = nullptr, *ys = nullptr, *zs = nullptr;  // [n] sorted, wrapped
+    double* qs = nullptr;                                // [n] sorted charges (per call)
+};
+
+// real-space kernel constants (eq. 20/21)
+struct RealConst {
+    double a, xi, two_a, c64, rc2, R0, inv_eps;
+    double two_xi_sqrtpi;   // 2 xi / sqrt(pi)
+    double t_lin, t_quad;   // small-r Taylor: R ~ R0 - t_lin r + t_quad r^2
+    double r_small;         // below this the Taylor form is used
+};
+
+// wave-space constants (eq. 25-27)
+struct WaveConst {
+    int Ng[3];
+    int Nxh;            // Ng[0]/2+1
+    int P;
+    double L[3], h[3], inv_h[3];
+    double aw;          // Gaussian exponent in grid units: exp(-aw u^2), aw = 2 pi / P
+    double kfac[3];     // 2 pi / L_d
+    double gexp[3];     // (1-eta_d)/(4 xi^2)
+    double a;           // bead radius (shape factor j0(ka))
+    double scale_norm;  // c_n^2 h^3 / (eps N_tot)
+    double grad_fac[3]; // 2 alpha_w,d h_d = 4 pi /(P h_d): dW/dx_alpha = grad_fac * u * W
+};
+
+enum Pass { PASS_CELLS = 0, PASS_REAL, PASS_SPREAD, PASS_FFT, PASS_SCALE, PASS_IFFT, PASS_GATHER, PASS_KRYLOV, PASS_OTHER, PASS_COUNT };
+
+struct pce_ctx {
+    pce_params p;
+    cudaStream_t st = nullptr;
+    std::string err;
+    RealConst rk;
+    WaveConst wk;
+    double V = 0, eta[3], h[3];
+    double kconst = 0;  // 1/(4 xi^2 V eps)
+
+    int N = 0, Nbead = 0, Nbody = 0, Nion = 0;
+    bool have_system = false;
+    std::vector<int> body_off_h;
+
+    double *x = nullptr, *y = nullptr, *z = nullptr;     // [N] wrapped, caller order
+    int* body_off = nullptr;                             // [Nbody+1]
+    int* body_of = nullptr;                              // [Nbead]
+    double *rx = nullptr, *ry = nullptr, *rz = nullptr;  // [Nbead] r_ij
+    double *X = nullptr, *Y = nullptr, *Z = nullptr;     // [Nbody] centres (unwrapped about first bead)
+
+    Bins all, bead;
+    int* scan_tmp = nullptr;  // block sums for the scans
+    size_t scan_tmp_n = 0;
+
+    // cached bead-bead near field (CSR over the bead binning's sorted order)
+    int* csr_ptr = nullptr;
+    int* csr_col = nullptr;
+    double* csr_val = nullptr;
+    long long nnz = 0, nnz_cap = 0;
+
+    // mesh
+    double* grid = nullptr;
+    cufftDoubleComplex* gridk = nullptr;
+    cufftHandle planF = 0, planB = 0;
+    void* fft_work = nullptr;
+    bool have_plans = false;
+
+    // per-call work vectors
+    double *w_real = nullptr, *w_wave = nullptr;            // [N] sorted-order potentials
+    double *w_ex = nullptr, *w_ey = nullptr, *w_ez = nullptr;  // [N] sorted-order real-space field
+    double *w_kx = nullptr, *w_ky = nullptr, *w_kz = nullptr;  // [N] sorted-order wave-space field
+    double* scal = nullptr;  // device scalars
+    // Krylov vectors [Nbead]
+    double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr, *cg_rhs = nullptr;
+    double *ev_psi = nullptr, *ev_ex = nullptr, *ev_ey = nullptr, *ev_ez = nullptr;  // [N]
+    double* cg_scal = nullptr;  // [3*(max_iter+2)]
+    // host staging for pce_step_host
+    double* hs_dev = nullptr;
+    size_t hs_dev_n = 0;
+
+    long long bytes = 0;
+    long long launches = 0;
+
+    // timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    struct Rec { int pass; cudaEvent_t a, b; };
+    std::vector<Rec> recs;
+    pce_timings tm;
+};
+
+// ---------------------------------------------------------------- helpers
+#define PCE_CUDA(ctx, call)                                                            \
+    do {                                                                               \
+        cudaError_t e__ = (call);                                                      \
+        if (e__ != cudaSuccess) {                                                      \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);           \
+            return PCE_ECUDA;                                                          \
+        }                                                                              \
+    } while (0)
+
+static inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+struct PassTimer {
+    pce_ctx* c;
+    int pass;
+    cudaEvent_t a = nullptr, b = nullptr;
+    PassTimer(pce_ctx* ctx, int pass_) : c(ctx), pass(pass_) {
+        if (!c->timing) return;
+        while (c->ev_used + 2 > c->ev_pool.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            c->ev_pool.push_back(e);
+        }
+        a = c->ev_pool[c->ev_used++];
+        b = c->ev_pool[c->ev_used++];
+        cudaEventRecord(a, c->st);
+    }
+    ~PassTimer() {
+        if (!c->timing) return;
+        cudaEventRecord(b, c->st);
+        c->recs.push_back({pass, a, b});
+    }
+};
+
+// cells.cu
+int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3]);
+void bins_free(Bins& b);
+int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const double* z);
+int exclusive_scan(pce_ctx* c, int* data, int n_plus_1);  // in place over n+1 entries (last input must be 0)
+int wrap_positions(pce_ctx* c, int n, const double* xi, const double* yi, const double* zi, double* xo, double* yo, double* zo);
+int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out);
+
+// realspace.cu
+int real_direct(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+int real_csr_build(pce_ctx* c, const Bins& b);
+int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s);
+
+// wave.cu
+int wave_spread(pce_ctx* c, const Bins& b);
+int wave_fft_scale_ifft(pce_ctx* c);
+int wave_gather(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+
+// krylov.cu
+int bodies_setup(pce_ctx* c);
+int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
+int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
+               double* S, double* U_body, double* U_tot, double* psi_out);
+
+// pce_api.cu
+int op_matvec_bead(pce_ctx* c, const double* q, double* psi);
+int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez);

@@ -1,0 +1,252 @@
+// realspace.cu -- real-space part of the Ewald split (eq. 19 second line):
+// the closed-form pair kernel eq. 20, its r -> 0 limit
+// eq. 21 and its derivative (not printed in the paper; derived
+// in DESIGN.md "Real-space kernel"), summed over linked-cell neighbours
+// (PAPER.md:200, 262).  Two uses: a direct pass (potential, optionally field)
+// and a cached CSR near field for the bead-only solver matvec, positions
+// being frozen during a Krylov solve.
+#include "pce_internal.h"
+
+struct CellGeom {
+    int nc[3], range[3];
+    double L[3], inv_cell[3];
+};
+
+static CellGeom geom_of(const Bins& b)
+{
+    CellGeom g;
+    for (int d = 0; d < 3; ++d) {
+        g.nc[d] = b.nc[d]; g.range[d] = b.range[d]; g.L[d] = b.L[d]; g.inv_cell[d] = b.nc[d] / b.L[d];
+    }
+    return g;
+}
+
+// F(u) = (2 xi^2 u^2 + 1) erfc(u xi) - (2 xi/sqrt(pi)) u exp(-u^2 xi^2), u >= 0.
+// eq. 20's six exp/erfc terms are c64/r [F(r+2a) + F(r-2a) - 2F(r)], c64 = 1/(64 pi a^2 xi^2);
+// for r < 2a, F(r-2a) = 2(2 xi^2 (r-2a)^2 + 1) - F(2a-r) and the polynomial part
+// cancels the Heaviside term up to 2 c64 / r.
+__device__ __forceinline__ void F_and_dF(double u, double xi, double& F, double& dF)
+{
+    const double x = u * xi;
+    const double e = exp(-x * x);
+    const double ecx = erfcx(x);
+    const double isp = 0.56418958354775628695;  // 1/sqrt(pi)
+    F = e * ((2.0 * x * x + 1.0) * ecx - 2.0 * isp * x);
+    dF = xi * e * (4.0 * x * ecx - 4.0 * isp);
+}
+
+// R(r) and dR/dr for r > 0 (times eps_f)
+__device__ __forceinline__ void pair_kernel(const RealConst& k, double r, double& R, double& dR)
+{
+    if (r < k.r_small) {
+        R = k.R0 - k.t_lin * r + k.t_quad * r * r;
+        dR = -k.t_lin + 2.0 * k.t_quad * r;
+        return;
+    }
+    double Fp, dFp, Fm, dFm, Fr, dFr;
+    F_and_dF(r + k.two_a, k.xi, Fp, dFp);
+    F_and_dF(fabs(r - k.two_a), k.xi, Fm, dFm);
+    F_and_dF(r, k.xi, Fr, dFr);
+    const double B = (r >= k.two_a) ? (Fp + Fm - 2.0 * Fr) : (Fp - Fm - 2.0 * Fr + 2.0);
+    const double dB = dFp + dFm - 2.0 * dFr;
+    const double ir = 1.0 / r;
+    R = k.c64 * B * ir;
+    dR = k.c64 * ir * (dB - B * ir);
+}
+
+__device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+// visit every (neighbour j, image) of sorted particle i with r < r_c
+template <class Op>
+__device__ __forceinline__ void for_neighbors(const CellGeom& g, const int* __restrict__ cell_start, const double* __restrict__ xs,
+                                              const double* __restrict__ ys, const double* __restrict__ zs, int i, double rc2, Op& op)
+{
+    const double xi = xs[i], yi = ys[i], zi = zs[i];
+    const int cx = min((int)(xi * g.inv_cell[0]), g.nc[0] - 1);
+    const int cy = min((int)(yi * g.inv_cell[1]), g.nc[1] - 1);
+    const int cz = min((int)(zi * g.inv_cell[2]), g.nc[2] - 1);
+    for (int oz = -g.range[2]; oz <= g.range[2]; ++oz) {
+        int nz = cz + oz;
+        const int wz = floor_div(nz, g.nc[2]);
+        nz -= wz * g.nc[2];
+        const double sz = wz * g.L[2];
+        for (int oy = -g.range[1]; oy <= g.range[1]; ++oy) {
+            int ny = cy + oy;
+            const int wy = floor_div(ny, g.nc[1]);
+            ny -= wy * g.nc[1];
+            const double sy = wy * g.L[1];
+            for (int ox = -g.range[0]; ox <= g.range[0]; ++ox) {
+                int nx = cx + ox;
+                const int wx = floor_div(nx, g.nc[0]);
+                nx -= wx * g.nc[0];
+                const double sx = wx * g.L[0];
+                const int cell = (nz * g.nc[1] + ny) * g.nc[0] + nx;
+                const int jb = cell_start[cell], je = cell_start[cell + 1];
+                const bool home = (ox == 0 && oy == 0 && oz == 0);
+                for (int j = jb; j < je; ++j) {
+                    if (home && j == i) continue;  // beta = alpha, n = 0: the self term (eq. 21)
+                    const double dx = xi - (xs[j] + sx), dy = yi - (ys[j] + sy), dz = zi - (zs[j] + sz);
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 < rc2) op(j, dx, dy, dz, r2);
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- direct pass
+struct OpDirect {
+    const RealConst& k;
+    const double* __restrict__ qs;
+    bool field;
+    double psi = 0, ex = 0, ey = 0, ez = 0;
+    __device__ OpDirect(const RealConst& k_, const double* q_, bool f) : k(k_), qs(q_), field(f) {}
+    __device__ __forceinline__ void operator()(int j, double dx, double dy, double dz, double r2)
+    {
+        const double q = qs[j];
+        if (r2 == 0.0) { psi += k.R0 * q; return; }  // coincident distinct particles: limit value, no field
+        const double r = sqrt(r2);
+        double R, dR;
+        pair_kernel(k, r, R, dR);
+        psi += R * q;
+        if (field) {
+            const double f = -dR * q / r;
+            ex += f * dx; ey += f * dy; ez += f * dz;
+        }
+    }
+};
+
+__global__ void __launch_bounds__(128)
+k_real_direct(int n, CellGeom g, RealConst k, const int* __restrict__ cell_start, const double* __restrict__ xs,
+              const double* __restrict__ ys, const double* __restrict__ zs, const double* __restrict__ qs, int field,
+              double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey, double* __restrict__ ez)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    OpDirect op(k, qs, field != 0);
+    for_neighbors(g, cell_start, xs, ys, zs, i, k.rc2, op);
+    psi[i] = (op.psi + k.R0 * qs[i]) * k.inv_eps;  // + self term, eq. 21
+    if (field) {
+        ex[i] = op.ex * k.inv_eps; ey[i] = op.ey * k.inv_eps; ez[i] = op.ez * k.inv_eps;
+    }
+}
+
+int real_direct(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s)
+{
+    if (b.n == 0) return PCE_OK;
+    PassTimer t(c, PASS_REAL);
+    k_real_direct<<<cdiv(b.n, 128), 128, 0, c->st>>>(b.n, geom_of(b), c->rk, b.cell_start, b.xs, b.ys, b.zs, b.qs, field ? 1 : 0,
+                                                     psi_s, ex_s, ey_s, ez_s);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+// ---------------------------------------------------------------- cached near field (CSR)
+struct OpCount {
+    int cnt = 0;
+    __device__ __forceinline__ void operator()(int, double, double, double, double) { ++cnt; }
+};
+
+__global__ void __launch_bounds__(128)
+k_csr_count(int n, CellGeom g, double rc2, const int* __restrict__ cell_start, const double* __restrict__ xs,
+            const double* __restrict__ ys, const double* __restrict__ zs, int* __restrict__ row_ptr)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    OpCount op;
+    for_neighbors(g, cell_start, xs, ys, zs, i, rc2, op);
+    row_ptr[i] = op.cnt + 1;  // + the diagonal (self term)
+}
+
+struct OpFill {
+    const RealConst& k;
+    int* __restrict__ col;
+    double* __restrict__ val;
+    long long pos;
+    __device__ OpFill(const RealConst& k_, int* c_, double* v_, long long p_) : k(k_), col(c_), val(v_), pos(p_) {}
+    __device__ __forceinline__ void operator()(int j, double, double, double, double r2)
+    {
+        double R = k.R0, dR;
+        if (r2 > 0.0) pair_kernel(k, sqrt(r2), R, dR);
+        col[pos] = j;
+        val[pos] = R * k.inv_eps;
+        ++pos;
+    }
+};
+
+__global__ void __launch_bounds__(128)
+k_csr_fill(int n, CellGeom g, RealConst k, const int* __restrict__ cell_start, const double* __restrict__ xs,
+           const double* __restrict__ ys, const double* __restrict__ zs, const int* __restrict__ row_ptr,
+           int* __restrict__ col, double* __restrict__ val)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long pos = row_ptr[i];
+    col[pos] = i;
+    val[pos] = k.R0 * k.inv_eps;  // self term, eq. 21
+    OpFill op(k, col, val, pos + 1);
+    for_neighbors(g, cell_start, xs, ys, zs, i, k.rc2, op);
+}
+
+int real_csr_build(pce_ctx* c, const Bins& b)
+{
+    c->nnz = 0;
+    if (b.n == 0) return PCE_OK;
+    PassTimer t(c, PASS_REAL);
+    const int n = b.n;
+    PCE_CUDA(c, cudaMemsetAsync(c->csr_ptr + n, 0, sizeof(int), c->st));
+    k_csr_count<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk.rc2, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr);
+    c->launches++;
+    int rc = exclusive_scan(c, c->csr_ptr, n + 1);
+    if (rc) return rc;
+    int nnz = 0;
+    PCE_CUDA(c, cudaMemcpyAsync(&nnz, c->csr_ptr + n, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    PCE_CUDA(c, cudaStreamSynchronize(c->st));
+    if (nnz < 0) { c->err = "near-field entry count overflows int32"; return PCE_ENOMEM; }
+    if (nnz > c->nnz_cap) {
+        cudaFree(c->csr_col); cudaFree(c->csr_val);
+        c->csr_col = nullptr; c->csr_val = nullptr;
+        c->bytes -= c->nnz_cap * 12;
+        c->nnz_cap = (long long)(nnz * 1.1) + 1024;
+        if (cudaMalloc(&c->csr_col, c->nnz_cap * sizeof(int)) != cudaSuccess ||
+            cudaMalloc(&c->csr_val, c->nnz_cap * sizeof(double)) != cudaSuccess) {
+            c->err = "out of device memory for the cached near field";
+            c->nnz_cap = 0;
+            return PCE_ENOMEM;
+        }
+        c->bytes += c->nnz_cap * 12;
+    }
+    c->nnz = nnz;
+    k_csr_fill<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr, c->csr_col,
+                                                c->csr_val);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+// one warp per row; x = b.qs (sorted charges), y = psi_s (sorted)
+__global__ void __launch_bounds__(256)
+k_csr_spmv(int n, const int* __restrict__ row_ptr, const int* __restrict__ col, const double* __restrict__ val,
+           const double* __restrict__ x, double* __restrict__ y)
+{
+    const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (row >= n) return;
+    const int b = row_ptr[row], e = row_ptr[row + 1];
+    double s = 0.0;
+    for (int k = b + lane; k < e; k += 32) s += val[k] * x[col[k]];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    if (lane == 0) y[row] = s;
+}
+
+int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s)
+{
+    if (b.n == 0) return PCE_OK;
+    PassTimer t(c, PASS_REAL);
+    k_csr_spmv<<<cdiv((long long)b.n * 32, 256), 256, 0, c->st>>>(b.n, c->csr_ptr, c->csr_col, c->csr_val, b.qs, psi_s);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
