@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path on synthetic inputs.
+
+One "step" = cell lists + cached near field, the induced-charge Krylov solve (eq. 13), the final
+potential+field evaluation, forces / torques / energies -- i.e. set_positions + solve + forces through the
+C ABI.  metric = Ewald operator applications per second over whole steps (bead-only solver matvecs plus full
+evaluations), ms_per_step = induced-charge solve ms/step (BASELINE.json's two headline numbers).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+N > 1 (torchrun): the path does not shard (replicas only) -- every rank runs an
+independent replica with its own seed; value is the sum over ranks, time the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "ewald_matvecs_per_s", "matvec/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config index 1..5 (default 5: 500k beads + 1M ions)")
+    ap.add_argument("--tol", type=float, default=1e-10, help="Ewald tolerance (xi, r_c, P follow eqs. 23, 28, 32)")
+    ap.add_argument("--P", type=int, default=0)
+    ap.add_argument("--tol-solver", type=float, default=1e-12)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-samples", type=int, nargs=2, default=None, help="two target counts for the oracle timing")
+    return ap.parse_args()
+
+
+def make_workload(idx, rank=0):
+    import workloads as wl
+    seed = wl.configs.BASE_SEED + idx + 1000 * rank
+    if idx == 1:
+        return wl.config1()
+    if idx == 2:
+        return wl.config2(d=3.0, seed=seed)
+    if idx == 3:
+        return wl.config3(seed=seed)
+    if idx == 4:
+        return wl.config4(seed=seed)
+    return wl.config5(seed=seed)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+# ---------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, dev):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(dev), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "200"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, reasons = [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[0])); out["sm_max_mhz"] = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if "Active" in v and "Not" not in v:
+                    reasons.add(name)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+        out["reasons"] = sorted(reasons)
+        out["samples"] = len(sm)
+        return out
+
+
+# ---------------------------------------------------------------- oracle timing (cpu_baseline / --impl reference)
+def oracle_matvec_seconds(w, samples, flavour="bead", seed=0):
+    """Time the oracle (as it stands) on a bounded sample: potentials (flavour 'bead': bead sources and
+    targets, potential only; 'full': all particles, potential + field) at S1 and S2 random targets from
+    ALL sources; t(S) = A + B S is extrapolated to every target.  Small configs are timed in full."""
+    import oracle as orc
+    rng = np.random.default_rng(seed)
+    if flavour == "bead":
+        x, field = w.x[:w.N_bead], False
+    else:
+        x, field = w.x, True
+    n = x.shape[0]
+    q = rng.normal(size=n)
+    if n <= 3000:
+        t0 = time.perf_counter()
+        orc.ewald_eval(x, q, w.L, w.a, w.eps_f, field=field)
+        dt = time.perf_counter() - t0
+        return dt, f"full {flavour} matvec, {n} targets", dt
+    ts = []
+    for S in samples:
+        tg = rng.choice(n, size=S, replace=False)
+        t0 = time.perf_counter()
+        orc.ewald_eval(x, q, w.L, w.a, w.eps_f, targets=tg, field=field)
+        ts.append(time.perf_counter() - t0)
+    B = (ts[1] - ts[0]) / (samples[1] - samples[0])
+    A = ts[0] - B * samples[0]
+    if B <= 0:  # noise: fall back to proportional scaling of the larger sample
+        A, B = 0.0, ts[1] / samples[1]
+    full = max(A, 0.0) + B * n
+    return full, f"{flavour} matvec at {samples[0]} and {samples[1]} of {n} targets from all {n} sources, t = A + B*S extrapolated to {n}", sum(ts)
+
+
+def default_samples(w):
+    # at least 4x the core count: the oracle parallelises over targets
+    if w.N > 500000:
+        return (64, 192)
+    if w.N > 50000:
+        return (128, 384)
+    return (256, 768)
+
+
+def run_reference(args, rank, world):
+    """The oracle timed on the host cores (the reference arm of this tier).  Rank 0 only."""
+    if rank != 0:
+        return
+    import oracle as orc
+    orc.build()
+    w = make_workload(args.config)
+    samples = tuple(args.cpu_samples) if args.cpu_samples else default_samples(w)
+    secs = []
+    for i in range(args.warmup + args.steps):
+        full, desc, spent = oracle_matvec_seconds(w, samples, "bead" if w.N_bead else "full", seed=i)
+        if i >= args.warmup:
+            secs.append(full)
+        if spent > 60 and i == 0 and args.warmup > 0:  # keep the whole run within minutes
+            args.warmup = 0
+            secs.append(full)
+    t = float(np.mean(secs))
+    val = 1.0 / t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "grid": [int(g) for g in w.Ng]},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import paper_2401_04865_b200 as pce
+
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        pce.build()
+    if dist:
+        dist.barrier()
+    w = make_workload(args.config, rank)
+    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    info = ctx.info()
+    hbm_peak, peak_src, _ = peaks()
+    grid_bytes = 8 * int(np.prod(w.Ng))
+    l2_flush = None
+    if grid_bytes < 256 << 20:  # working set may sit in the 126 MB L2: flush between timed steps
+        l2_flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def step(timed):
+        ctx.set_positions(x, y, z)
+        t_cells = ctx.timings() if timed else None
+        q, Phi, sinfo = ctx.solve(Q, qi, w.E0, allow_noconv=True)
+        t_solve = ctx.timings() if timed else None
+        out = ctx.forces(q, w.E0)
+        t_force = ctx.timings() if timed else None
+        return q, out, sinfo, (t_cells, t_solve, t_force)
+
+    for _ in range(args.warmup):
+        step(False)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    ctx.set_timing(True)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = ctx.launch_count()
+    acc = {}
+    ms_steps, ms_solve, iters, n_m1, n_m2 = [], [], [], 0, 0
+    for _ in range(args.steps):
+        if l2_flush is not None:
+            l2_flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        q, out, sinfo, tms = step(True)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_steps.append(e0.elapsed_time(e1))
+        for t in tms:
+            for k, v in t.items():
+                acc[k] = acc.get(k, 0) + v
+        ms_solve.append(tms[1]["total"])
+        iters.append(sinfo["iters"])
+        n_m1 += tms[1]["n_matvec_bead"]
+        n_m2 += tms[1]["n_eval_full"] + tms[2]["n_eval_full"]
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    ctx.set_timing(False)
+    total_ms = float(sum(ms_steps))
+    n_apply = n_m1 + n_m2
+    if dist:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        cnt = torch.tensor([n_apply], dtype=torch.float64, device="cuda")
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+        n_apply_all = float(cnt.item())
+    else:
+        n_apply_all = float(n_apply)
+    value = n_apply_all / (total_ms * 1e-3)
+
+    # ---- end to end through the host-buffer call (H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        def pin(a):
+            return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
+        hx, hy, hz = pin(w.x[:, 0]), pin(w.x[:, 1]), pin(w.x[:, 2])
+        hQ, hqi = pin(w.Q_body), pin(w.q_ion)
+        nb = w.N_body
+        outb = {"q": pin(np.zeros(w.N)), "Phi": pin(np.zeros(max(nb, 1))), "fx": pin(np.zeros(w.N)), "fy": pin(np.zeros(w.N)),
+                "fz": pin(np.zeros(w.N)), "F": pin(np.zeros(max(3 * nb, 1))), "T": pin(np.zeros(max(3 * nb, 1))),
+                "S": pin(np.zeros(max(3 * nb, 1))), "U": pin(np.zeros(3))}
+        ctx.step_host(hx, hy, hz, hQ, hqi, w.E0, outb)  # warm
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        t0 = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        n_e2e = 0
+        for _ in range(args.steps):
+            si = ctx.step_host(hx, hy, hz, hQ, hqi, w.E0, outb)
+            n_e2e += si["matvecs"] + 1
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))  # the call is synchronous: host clock bounds it
+        if dist:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+            cnt = torch.tensor([n_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+            n_e2e = float(cnt.item())
+        e2e = {"value": n_e2e / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * (3 * w.N + nb + w.N_ion),
+               "d2h_bytes_per_step": 8 * (w.N + nb + 3 * w.N + 9 * nb + 3), "ms_per_step": ms / args.steps}
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    # ---- per-pass rooflines (algorithmic bytes of SURVEY.md 8(d), stated in DESIGN.md)
+    Ng3, Nk = int(np.prod(w.Ng)), int((w.Ng[0] // 2 + 1) * w.Ng[1] * w.Ng[2])
+    nm1, nfull = max(acc["n_matvec_bead"], 1), max(acc["n_eval_full"], 1)
+    npairs = max(acc["n_fft_pairs"], 1)
+
+    def rf(ms_total, launches_, bytes_per_launch, bound="hbm"):
+        if ms_total <= 0:
+            return None
+        gbs = bytes_per_launch / (ms_total / launches_ * 1e-3) / 1e9
+        return {"bound": bound, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                "ms_per_launch": ms_total / launches_, "algorithmic_bytes": bytes_per_launch, "launches": launches_}
+    passes = {
+        "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3),
+        "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead),
+        "real_bead_csr": rf(acc["bead_real"], nm1, 12 * info["nnz_near"] + 20 * w.N_bead),
+        "scale": rf(acc["scale"], npairs, 32 * Nk),
+        "fft_d2z(cuFFT)": rf(acc["fft"], npairs, 8 * Ng3 + 16 * Nk),
+        "ifft_z2d(cuFFT)": rf(acc["ifft"], npairs, 8 * Ng3 + 16 * Nk),
+        "spread_full": rf(acc["spread"] - acc["bead_spread"], nfull, 32 * w.N + 8 * Ng3),
+        "gather_full_field": rf(acc["gather"] - acc["bead_gather"], nfull, 8 * Ng3 + 64 * w.N),
+    }
+    own = {k: v for k, v in passes.items() if v and "cuFFT" not in k}
+    dom = max(own, key=lambda k: own[k]["ms_per_launch"] * own[k]["launches"])
+    roof = dict(own[dom])
+    roof["kernel"] = dom
+    roof["peak_source"] = peak_src
+    roof["traffic"] = None  # dram bytes from ncu: see profiles/
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "N_body": w.N_body, "grid": [int(g) for g in w.Ng],
+                   "P": int(ctx.params.P), "xi": ctx.params.xi, "rc": ctx.params.rc, "ewald_tol": args.tol,
+                   "solver_tol": args.tol_solver, "cells": info["ncell"], "nnz_near": info["nnz_near"],
+                   "l2": "flushed between timed steps" if l2_flush is not None else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
+                   "multi_gpu": "replicas only"},
+        "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
+                  "evals_full": acc["n_eval_full"], "rel_resid": sinfo["rel_resid"], "converged": sinfo["converged"]},
+        "passes_ms_per_step": {k: acc[k] / args.steps for k in ("cells", "real", "spread", "fft", "scale", "ifft", "gather", "krylov", "other", "total")},
+        "roofline": roof, "roofline_passes": passes, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+    }
+    if not args.no_cpu_baseline:
+        import oracle as orc
+        orc.build()
+        samples = tuple(args.cpu_samples) if args.cpu_samples else default_samples(w)
+        t1, d1, _ = oracle_matvec_seconds(w, samples, "bead" if w.N_bead else "full")
+        line["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": d1,
+                                "seconds_per_matvec": t1}
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

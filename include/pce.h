@@ -82,7 +82,10 @@ typedef struct {
  * call that ran with timing enabled (pce_set_timing). */
 typedef struct {
     double cells, real, spread, fft, scale, ifft, gather, krylov, other, total;
-    int    n_matvec_bead, n_eval_full;
+    /* the share of real / spread / gather spent in bead-only solver matvecs
+     * (the rest belongs to full evaluations and the near-field build) */
+    double bead_real, bead_spread, bead_gather;
+    int    n_matvec_bead, n_eval_full, n_fft_pairs;
 } pce_timings;
 
 /* Derived quantities, for reports and tests. */

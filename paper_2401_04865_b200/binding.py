@@ -37,7 +37,8 @@ class PceSolveInfo(C.Structure):
 
 class PceTimings(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("cells", "real", "spread", "fft", "scale", "ifft", "gather", "krylov", "other", "total")] + \
-               [("n_matvec_bead", C.c_int), ("n_eval_full", C.c_int)]
+               [(n, C.c_double) for n in ("bead_real", "bead_spread", "bead_gather")] + \
+               [("n_matvec_bead", C.c_int), ("n_eval_full", C.c_int), ("n_fft_pairs", C.c_int)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

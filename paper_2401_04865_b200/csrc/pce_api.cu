@@ -53,6 +53,11 @@ static void timing_end(pce_ctx* c)
         cudaEventElapsedTime(&ms, r.a, r.b);
         *slot[r.pass] += ms;
         c->tm.total += ms;
+        if (r.bead) {
+            if (r.pass == PASS_REAL) c->tm.bead_real += ms;
+            if (r.pass == PASS_SPREAD) c->tm.bead_spread += ms;
+            if (r.pass == PASS_GATHER) c->tm.bead_gather += ms;
+        }
     }
     c->recs.clear();
     c->ev_used = 0;
@@ -337,12 +342,17 @@ static int apply_operator(pce_ctx* c, Bins& b, bool use_csr, const double* q, do
 int op_matvec_bead(pce_ctx* c, const double* q, double* psi)
 {
     c->tm.n_matvec_bead++;
-    return apply_operator(c, c->bead, true, q, psi, nullptr, nullptr, nullptr);
+    c->tm.n_fft_pairs++;
+    c->in_bead_matvec = true;
+    int rc = apply_operator(c, c->bead, true, q, psi, nullptr, nullptr, nullptr);
+    c->in_bead_matvec = false;
+    return rc;
 }
 
 int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
 {
     c->tm.n_eval_full++;
+    c->tm.n_fft_pairs++;
     return apply_operator(c, c->all, false, q, psi, Ex, Ey, Ez);
 }
 

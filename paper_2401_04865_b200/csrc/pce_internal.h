@@ -112,7 +112,8 @@ struct pce_ctx {
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
     size_t ev_used = 0;
-    struct Rec { int pass; cudaEvent_t a, b; };
+    struct Rec { int pass; bool bead; cudaEvent_t a, b; };
+    bool in_bead_matvec = false;
     std::vector<Rec> recs;
     pce_timings tm;
 };
@@ -147,7 +148,7 @@ struct PassTimer {
     ~PassTimer() {
         if (!c->timing) return;
         cudaEventRecord(b, c->st);
-        c->recs.push_back({pass, a, b});
+        c->recs.push_back({pass, c->in_bead_matvec, a, b});
     }
 };
 
