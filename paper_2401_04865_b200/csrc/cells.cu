@@ -127,14 +127,14 @@ int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double*
 
 // ---------------------------------------------------------------- binning
 __global__ void k_cell_count(int n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
-                             int ncx, int ncy, int ncz, double sx, double sy, double sz, int* __restrict__ cell_of,
-                             int* __restrict__ count)
+                             int ncx, int ncy, int ncz, double sx, double sy, double sz, int mx, int my, int mz, int dvx, int dvy,
+                             int dvz, int* __restrict__ cell_of, int* __restrict__ count)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    int cx = min((int)(x[i] * sx), ncx - 1);
-    int cy = min((int)(y[i] * sy), ncy - 1);
-    int cz = min((int)(z[i] * sz), ncz - 1);
+    int cx = min(min((int)(x[i] * sx), mx) / dvx, ncx - 1);
+    int cy = min(min((int)(y[i] * sy), my) / dvy, ncy - 1);
+    int cz = min(min((int)(z[i] * sz), mz) / dvz, ncz - 1);
     const int cidx = (cz * ncy + cy) * ncx + cx;
     cell_of[i] = cidx;
     atomicAdd(&count[cidx], 1);
@@ -172,11 +172,13 @@ __global__ void k_iota(int n, int* p)
 }
 
 __global__ void k_gather3(int n, const int* __restrict__ perm, const double* __restrict__ x, const double* __restrict__ y,
-                          const double* __restrict__ z, double* __restrict__ xs, double* __restrict__ ys, double* __restrict__ zs)
+                          const double* __restrict__ z, double* __restrict__ xs, double* __restrict__ ys, double* __restrict__ zs,
+                          int* __restrict__ inv)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int j = perm[i];
+    inv[j] = i;
     xs[i] = x[j]; ys[i] = y[j]; zs[i] = z[j];
 }
 
@@ -184,7 +186,10 @@ int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3])
 {
     bins_free(b);
     b.n = n;
-    for (int d = 0; d < 3; ++d) { b.nc[d] = nc[d]; b.range[d] = range[d]; b.L[d] = c->p.L[d]; }
+    for (int d = 0; d < 3; ++d) {
+        b.nc[d] = nc[d]; b.range[d] = range[d]; b.L[d] = c->p.L[d];
+        b.scale[d] = nc[d] / c->p.L[d]; b.imax[d] = nc[d] - 1; b.div[d] = 1;
+    }
     b.ncell = nc[0] * nc[1] * nc[2];
     const size_t ni = (size_t)(n > 0 ? n : 1);
     PCE_CUDA(c, cudaMalloc(&b.cell_of, ni * sizeof(int)));
@@ -192,17 +197,29 @@ int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3])
     PCE_CUDA(c, cudaMalloc(&b.cell_fill, ((size_t)b.ncell + 1) * sizeof(int)));
     PCE_CUDA(c, cudaMalloc(&b.perm, ni * sizeof(int)));
     PCE_CUDA(c, cudaMalloc(&b.perm_tmp, ni * sizeof(int)));
+    PCE_CUDA(c, cudaMalloc(&b.inv, ni * sizeof(int)));
     PCE_CUDA(c, cudaMalloc(&b.xs, ni * sizeof(double)));
     PCE_CUDA(c, cudaMalloc(&b.ys, ni * sizeof(double)));
     PCE_CUDA(c, cudaMalloc(&b.zs, ni * sizeof(double)));
     PCE_CUDA(c, cudaMalloc(&b.qs, ni * sizeof(double)));
-    c->bytes += (long long)(ni * (3 * 4 + 4 * 8) + ((size_t)b.ncell + 1) * 8);
+    c->bytes += (long long)(ni * (4 * 4 + 4 * 8) + ((size_t)b.ncell + 1) * 8);
+    return PCE_OK;
+}
+
+int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile)
+{
+    int nc[3], range[3] = {1, 1, 1};
+    for (int d = 0; d < 3; ++d) nc[d] = (c->p.Ng[d] + tile - 1) / tile;
+    int rc = bins_alloc(c, b, n, nc, range);
+    if (rc) return rc;
+    // the same 1/h the mesh kernels use, so that floor(x/h) agrees bit for bit
+    for (int d = 0; d < 3; ++d) { b.scale[d] = c->wk.inv_h[d]; b.imax[d] = c->p.Ng[d] - 1; b.div[d] = tile; }
     return PCE_OK;
 }
 
 void bins_free(Bins& b)
 {
-    cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp);
+    cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp); cudaFree(b.inv);
     cudaFree(b.xs); cudaFree(b.ys); cudaFree(b.zs); cudaFree(b.qs);
     b = Bins();
 }
@@ -224,8 +241,9 @@ int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const doub
     } else {
         PCE_CUDA(c, cudaMemsetAsync(b.cell_start, 0, ((size_t)b.ncell + 1) * sizeof(int), c->st));
         PCE_CUDA(c, cudaMemsetAsync(b.cell_fill, 0, ((size_t)b.ncell + 1) * sizeof(int), c->st));
-        k_cell_count<<<cdiv(n, 256), 256, 0, c->st>>>(n, x, y, z, b.nc[0], b.nc[1], b.nc[2], b.nc[0] / b.L[0],
-                                                      b.nc[1] / b.L[1], b.nc[2] / b.L[2], b.cell_of, b.cell_start);
+        k_cell_count<<<cdiv(n, 256), 256, 0, c->st>>>(n, x, y, z, b.nc[0], b.nc[1], b.nc[2], b.scale[0], b.scale[1], b.scale[2],
+                                                      b.imax[0], b.imax[1], b.imax[2], b.div[0], b.div[1], b.div[2], b.cell_of,
+                                                      b.cell_start);
         c->launches++;
         int rc = exclusive_scan(c, b.cell_start, b.ncell + 1);
         if (rc) return rc;
@@ -233,7 +251,7 @@ int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const doub
         k_cell_rank<<<cdiv((long long)b.ncell * 32, 256), 256, 0, c->st>>>(b.ncell, b.cell_start, b.perm_tmp, b.perm);
         c->launches += 2;
     }
-    k_gather3<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, x, y, z, b.xs, b.ys, b.zs);
+    k_gather3<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, x, y, z, b.xs, b.ys, b.zs, b.inv);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;

@@ -23,6 +23,11 @@ struct Bins {
     int ncell = 1;
     int range[3] = {1, 1, 1};  // stencil half width: 1 (cells) or image count
     double L[3];
+    // cell index per dimension = min(min((int)(x * scale), imax) / div, nc - 1):
+    //   real-space cells: scale = nc/L, div = 1;  mesh tiles: scale = 1/h, imax = Ng-1, div = tile edge
+    double scale[3] = {1, 1, 1};
+    int imax[3] = {0, 0, 0}, div[3] = {1, 1, 1};
+    int* inv = nullptr;         // [n] index in the subset -> sorted slot
     int* cell_of = nullptr;     // [n]
     int* cell_start = nullptr;  // [ncell+1]
     int* cell_fill = nullptr;   // [ncell+1] scratch
@@ -153,7 +158,8 @@ struct PassTimer {
 };
 
 // cells.cu
-int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3]);
+int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3]);          // real-space cells
+int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile);                                  // mesh tiles of `tile` grid points
 void bins_free(Bins& b);
 int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const double* z);
 int exclusive_scan(pce_ctx* c, int* data, int n_plus_1);  // in place over n+1 entries (last input must be 0)
