@@ -375,9 +375,9 @@ int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, doub
                                                        c->Y, c->Z, E0[0], E0[1], E0[2], e1, e2, Ub + nb);
         c->launches++;
         if (U_tot) {
-            if ((rc = sum_to(c, Ub, (long long)nb + c->Nion, c->scal + 4))) return rc;
-            if ((rc = sum_to(c, e1, N, c->scal + 5))) return rc;
-            if ((rc = sum_to(c, e2, N, c->scal + 6))) return rc;
+            if ((rc = sum_vector(c, Ub, nb + c->Nion, c->scal + 4))) return rc;
+            if ((rc = sum_vector(c, e1, N, c->scal + 5))) return rc;
+            if ((rc = sum_vector(c, e2, N, c->scal + 6))) return rc;
             k_energy_final<<<1, 1, 0, c->st>>>(c->scal + 4, U_tot);
             c->launches++;
         }

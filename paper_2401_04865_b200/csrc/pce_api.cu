@@ -68,7 +68,7 @@ static void free_system(pce_ctx* c)
 {
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z); cudaFree(c->body_off); cudaFree(c->body_of);
     cudaFree(c->rx); cudaFree(c->ry); cudaFree(c->rz); cudaFree(c->X); cudaFree(c->Y); cudaFree(c->Z);
-    bins_free(c->all); bins_free(c->bead);
+    bins_free(c->all); bins_free(c->bead); bins_free(c->wall); bins_free(c->wbead);
     cudaFree(c->csr_ptr); cudaFree(c->csr_col); cudaFree(c->csr_val);
     cudaFree(c->w_real); cudaFree(c->w_wave); cudaFree(c->w_ex); cudaFree(c->w_ey); cudaFree(c->w_ez);
     cudaFree(c->w_kx); cudaFree(c->w_ky); cudaFree(c->w_kz);
@@ -91,7 +91,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     cudaStreamSynchronize(c->st);
     free_system(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->scan_tmp);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -121,6 +121,7 @@ static int create_impl(pce_ctx* c)
     w.aw = 2.0 * PCE_PI / p.P;
     w.a = p.a;
     w.scale_norm = cn2 * h3 / (p.eps_f * ntot);
+    for (int r = 0; r < 32; ++r) w.G[r] = std::exp(-w.aw * r * r);
     RealConst& r = c->rk;
     r.a = p.a; r.xi = p.xi; r.two_a = 2.0 * p.a; r.inv_eps = 1.0 / p.eps_f;
     r.c64 = 1.0 / (64.0 * PCE_PI * p.a * p.a * p.xi * p.xi);
@@ -142,6 +143,7 @@ static int create_impl(pce_ctx* c)
     }
     c->bytes += (long long)(ng * 8 + nk * 16);
     PCE_CUDA(c, cudaMalloc(&c->scal, 64 * sizeof(double)));
+    PCE_CUDA(c, cudaMalloc(&c->sum_part, 1024 * sizeof(double)));
     // cuFFT plans sharing one work area
     size_t wsF = 0, wsB = 0;
     if (cufftCreate(&c->planF) != CUFFT_SUCCESS || cufftCreate(&c->planB) != CUFFT_SUCCESS) { c->err = "cufftCreate failed"; return PCE_ECUFFT; }
@@ -162,7 +164,7 @@ static int create_impl(pce_ctx* c)
     cufftSetWorkArea(c->planB, c->fft_work);
     cufftSetStream(c->planF, c->st);
     cufftSetStream(c->planB, c->st);
-    return PCE_OK;
+    return wave_tiles_init(c);
 }
 
 extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
@@ -218,6 +220,8 @@ static int positions_impl(pce_ctx* c, const double* x, const double* y, const do
         if ((rc = wrap_positions(c, c->N, x, y, z, c->x, c->y, c->z))) return rc;
         if ((rc = bins_build(c, c->all, c->x, c->y, c->z))) return rc;
         if ((rc = bins_build(c, c->bead, c->x, c->y, c->z))) return rc;  // beads are the first Nbead particles
+        if ((rc = bins_build(c, c->wall, c->x, c->y, c->z))) return rc;
+        if ((rc = bins_build(c, c->wbead, c->x, c->y, c->z))) return rc;
         if ((rc = bodies_setup(c))) return rc;
     }
     if ((rc = real_csr_build(c, c->bead))) return rc;
@@ -257,6 +261,8 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     cell_layout(c->p, nc, range);
     if ((rc = bins_alloc(c, c->all, N, nc, range))) return rc;
     if ((rc = bins_alloc(c, c->bead, c->Nbead, nc, range))) return rc;
+    if ((rc = bins_alloc_tiles(c, c->wall, N, 16))) return rc;
+    if ((rc = bins_alloc_tiles(c, c->wbead, c->Nbead, 16))) return rc;
     PCE_CUDA(c, cudaMalloc(&c->csr_ptr, ((size_t)c->Nbead + 2) * sizeof(int)));
     ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
     ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
@@ -282,57 +288,87 @@ extern "C" int pce_set_positions(pce_ctx* c, const double* x, const double* y, c
 }
 
 // ---------------------------------------------------------------- the operator
-__global__ void k_sum1(const double* __restrict__ in, int n, double* __restrict__ out)
+// out[0] = sum(in[0..n)): per-block partials, then one block (fixed order: deterministic)
+__global__ void __launch_bounds__(256) k_sum_partial(const double* __restrict__ in, int n, double* __restrict__ part)
 {
-    __shared__ double sh[32];
+    __shared__ double sh[8];
     double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) v += in[i];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) v += in[i];
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
     if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
     __syncthreads();
     if (threadIdx.x == 0) {
         double s = 0.0;
-        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += sh[i];
+        for (int i = 0; i < 8; ++i) s += sh[i];
+        part[blockIdx.x] = s;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_sum_final(const double* __restrict__ part, int nb, double* __restrict__ out)
+{
+    __shared__ double sh[8];
+    double v = 0.0;
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) v += part[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < 8; ++i) s += sh[i];
         out[0] = s;
     }
 }
 
-// psi[perm[i]] = real + wave - (sum q)/(4 xi^2 V eps); fields likewise (no constant)
-__global__ void k_finalize(int n, const int* __restrict__ perm, const double* __restrict__ re, const double* __restrict__ wa,
-                           const double* __restrict__ qsum, double kconst, double* __restrict__ psi, int field,
-                           const double* __restrict__ rx, const double* __restrict__ ry, const double* __restrict__ rz,
+int sum_vector(pce_ctx* c, const double* in, int n, double* out)
+{
+    int nb = cdiv(n, 256 * 8);
+    if (nb > 1024) nb = 1024;
+    if (nb < 1) nb = 1;
+    k_sum_partial<<<nb, 256, 0, c->st>>>(in, n, c->sum_part);
+    k_sum_final<<<1, 256, 0, c->st>>>(c->sum_part, nb, out);
+    c->launches += 2;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+// caller order j: psi[j] = real[inv_r[j]] + wave[inv_w[j]] - (sum q)/(4 xi^2 V eps); fields likewise (no constant)
+__global__ void k_finalize(int n, const int* __restrict__ inv_r, const int* __restrict__ inv_w, const double* __restrict__ re,
+                           const double* __restrict__ wa, const double* __restrict__ qsum, double kconst, double* __restrict__ psi,
+                           int field, const double* __restrict__ rx, const double* __restrict__ ry, const double* __restrict__ rz,
                            const double* __restrict__ kx, const double* __restrict__ ky, const double* __restrict__ kz,
                            double* __restrict__ ex, double* __restrict__ ey, double* __restrict__ ez)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int j = perm[i];
-    psi[j] = re[i] + wa[i] - kconst * qsum[0];
-    if (field) { ex[j] = rx[i] + kx[i]; ey[j] = ry[i] + ky[i]; ez[j] = rz[i] + kz[i]; }
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const int ir = inv_r[j], iw = inv_w[j];
+    psi[j] = re[ir] + wa[iw] - kconst * qsum[0];
+    if (field) { ex[j] = rx[ir] + kx[iw]; ey[j] = ry[ir] + ky[iw]; ez[j] = rz[ir] + kz[iw]; }
 }
 
-static int apply_operator(pce_ctx* c, Bins& b, bool use_csr, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
+// rb: real-space cells, wb: mesh tiles of the same particle subset
+static int apply_operator(pce_ctx* c, Bins& rb, Bins& wb, bool use_csr, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
 {
     const bool field = (Ex != nullptr);
-    const int n = b.n;
+    const int n = rb.n;
     int rc;
     {
         PassTimer t(c, PASS_OTHER);
-        if ((rc = gather_by_perm(c, n, b.perm, q, b.qs))) return rc;
-        k_sum1<<<1, 1024, 0, c->st>>>(q, n, c->scal);
-        c->launches++;
+        if ((rc = gather_by_perm(c, n, rb.perm, q, rb.qs))) return rc;
+        if ((rc = gather_by_perm(c, n, wb.perm, q, wb.qs))) return rc;
+        if ((rc = sum_vector(c, q, n, c->scal))) return rc;
     }
-    if (use_csr) rc = real_csr_spmv(c, b, c->w_real);                                   // step 1 (cached), eq. 20-21
-    else rc = real_direct(c, b, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);           // step 1, eq. 20-21
+    if (use_csr) rc = real_csr_spmv(c, rb, c->w_real);                                   // step 1 (cached), eq. 20-21
+    else rc = real_direct(c, rb, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);           // step 1, eq. 20-21
     if (rc) return rc;
-    if ((rc = wave_spread(c, b))) return rc;                                            // step 2, eq. 25
-    if ((rc = wave_fft_scale_ifft(c))) return rc;                                       // steps 3-5, eq. 26
-    if ((rc = wave_gather(c, b, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    if ((rc = wave_spread_tiles(c, wb))) return rc;                                      // step 2, eq. 25
+    if ((rc = wave_fft_scale_ifft(c))) return rc;                                        // steps 3-5, eq. 26
+    if ((rc = wave_gather_tiles(c, wb, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
     {
         PassTimer t(c, PASS_OTHER);
-        k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0, c->w_ex,
-                                                   c->w_ey, c->w_ez, c->w_kx, c->w_ky, c->w_kz, Ex, Ey, Ez);
+        k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, rb.inv, wb.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,
+                                                   c->w_ex, c->w_ey, c->w_ez, c->w_kx, c->w_ky, c->w_kz, Ex, Ey, Ez);
         c->launches++;
     }
     PCE_CUDA(c, cudaGetLastError());
@@ -344,7 +380,7 @@ int op_matvec_bead(pce_ctx* c, const double* q, double* psi)
     c->tm.n_matvec_bead++;
     c->tm.n_fft_pairs++;
     c->in_bead_matvec = true;
-    int rc = apply_operator(c, c->bead, true, q, psi, nullptr, nullptr, nullptr);
+    int rc = apply_operator(c, c->bead, c->wbead, true, q, psi, nullptr, nullptr, nullptr);
     c->in_bead_matvec = false;
     return rc;
 }
@@ -353,7 +389,7 @@ int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey
 {
     c->tm.n_eval_full++;
     c->tm.n_fft_pairs++;
-    return apply_operator(c, c->all, false, q, psi, Ex, Ey, Ez);
+    return apply_operator(c, c->all, c->wall, false, q, psi, Ex, Ey, Ez);
 }
 
 extern "C" int pce_matvec(pce_ctx* c, const double* q, double* psi)

@@ -57,6 +57,7 @@ struct WaveConst {
     double a;           // bead radius (shape factor j0(ka))
     double scale_norm;  // c_n^2 h^3 / (eps N_tot)
     double grad_fac[3]; // 2 alpha_w,d h_d = 4 pi /(P h_d): dW/dx_alpha = grad_fac * u * W
+    double G[32];       // exp(-aw r^2), r = 0..P-1
 };
 
 enum Pass { PASS_CELLS = 0, PASS_REAL, PASS_SPREAD, PASS_FFT, PASS_SCALE, PASS_IFFT, PASS_GATHER, PASS_KRYLOV, PASS_OTHER, PASS_COUNT };
@@ -80,7 +81,8 @@ struct pce_ctx {
     double *rx = nullptr, *ry = nullptr, *rz = nullptr;  // [Nbead] r_ij
     double *X = nullptr, *Y = nullptr, *Z = nullptr;     // [Nbody] centres (unwrapped about first bead)
 
-    Bins all, bead;
+    Bins all, bead;    // real-space linked cells (all particles / conductor beads)
+    Bins wall, wbead;  // mesh tiles (spread / gather)
     int* scan_tmp = nullptr;  // block sums for the scans
     size_t scan_tmp_n = 0;
 
@@ -102,6 +104,7 @@ struct pce_ctx {
     double *w_ex = nullptr, *w_ey = nullptr, *w_ez = nullptr;  // [N] sorted-order real-space field
     double *w_kx = nullptr, *w_ky = nullptr, *w_kz = nullptr;  // [N] sorted-order wave-space field
     double* scal = nullptr;  // device scalars
+    double* sum_part = nullptr;  // [1024] partial sums
     // Krylov vectors [Nbead]
     double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr, *cg_rhs = nullptr;
     double *ev_psi = nullptr, *ev_ex = nullptr, *ev_ey = nullptr, *ev_ez = nullptr;  // [N]
@@ -176,6 +179,11 @@ int wave_spread(pce_ctx* c, const Bins& b);
 int wave_fft_scale_ifft(pce_ctx* c);
 int wave_gather(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
 
+// wave_tiles.cu
+int wave_tiles_init(pce_ctx* c);
+int wave_spread_tiles(pce_ctx* c, const Bins& b);
+int wave_gather_tiles(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+
 // krylov.cu
 int bodies_setup(pce_ctx* c);
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
@@ -183,5 +191,6 @@ int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, doub
                double* S, double* U_body, double* U_tot, double* psi_out);
 
 // pce_api.cu
+int sum_vector(pce_ctx* c, const double* in, int n, double* out);  // deterministic two-stage sum
 int op_matvec_bead(pce_ctx* c, const double* q, double* psi);
 int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez);
