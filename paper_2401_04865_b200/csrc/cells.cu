@@ -221,6 +221,7 @@ void bins_free(Bins& b)
 {
     cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp); cudaFree(b.inv);
     cudaFree(b.xs); cudaFree(b.ys); cudaFree(b.zs); cudaFree(b.qs);
+    for (int d = 0; d < 3; ++d) { cudaFree(b.ws0[d]); cudaFree(b.we0[d]); cudaFree(b.we1[d]); }
     b = Bins();
 }
 

@@ -164,7 +164,7 @@ static int create_impl(pce_ctx* c)
     cufftSetWorkArea(c->planB, c->fft_work);
     cufftSetStream(c->planF, c->st);
     cufftSetStream(c->planB, c->st);
-    return wave_tiles_init(c);
+    return wave_bricks_init(c);
 }
 
 extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
@@ -222,6 +222,8 @@ static int positions_impl(pce_ctx* c, const double* x, const double* y, const do
         if ((rc = bins_build(c, c->bead, c->x, c->y, c->z))) return rc;  // beads are the first Nbead particles
         if ((rc = bins_build(c, c->wall, c->x, c->y, c->z))) return rc;
         if ((rc = bins_build(c, c->wbead, c->x, c->y, c->z))) return rc;
+        if ((rc = wave_window_coef(c, c->wall))) return rc;
+        if ((rc = wave_window_coef(c, c->wbead))) return rc;
         if ((rc = bodies_setup(c))) return rc;
     }
     if ((rc = real_csr_build(c, c->bead))) return rc;
@@ -261,8 +263,10 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     cell_layout(c->p, nc, range);
     if ((rc = bins_alloc(c, c->all, N, nc, range))) return rc;
     if ((rc = bins_alloc(c, c->bead, c->Nbead, nc, range))) return rc;
-    if ((rc = bins_alloc_tiles(c, c->wall, N, 16))) return rc;
-    if ((rc = bins_alloc_tiles(c, c->wbead, c->Nbead, 16))) return rc;
+    if ((rc = bins_alloc_tiles(c, c->wall, N, 8))) return rc;  // 8-point mesh bins = bricks of wave_bricks.cu
+    if ((rc = bins_alloc_tiles(c, c->wbead, c->Nbead, 8))) return rc;
+    if ((rc = wave_coef_alloc(c, c->wall))) return rc;
+    if ((rc = wave_coef_alloc(c, c->wbead))) return rc;
     PCE_CUDA(c, cudaMalloc(&c->csr_ptr, ((size_t)c->Nbead + 2) * sizeof(int)));
     ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
     ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
@@ -362,9 +366,9 @@ static int apply_operator(pce_ctx* c, Bins& rb, Bins& wb, bool use_csr, const do
     if (use_csr) rc = real_csr_spmv(c, rb, c->w_real);                                   // step 1 (cached), eq. 20-21
     else rc = real_direct(c, rb, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);           // step 1, eq. 20-21
     if (rc) return rc;
-    if ((rc = wave_spread_tiles(c, wb))) return rc;                                      // step 2, eq. 25
+    if ((rc = wave_spread_bricks(c, wb))) return rc;                                      // step 2, eq. 25
     if ((rc = wave_fft_scale_ifft(c))) return rc;                                        // steps 3-5, eq. 26
-    if ((rc = wave_gather_tiles(c, wb, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    if ((rc = wave_gather_bricks(c, wb, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
     {
         PassTimer t(c, PASS_OTHER);
         k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, rb.inv, wb.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,

@@ -35,6 +35,10 @@ struct Bins {
     int* perm_tmp = nullptr;    // [n]
     double *xs = nullptr, *ys = nullptr, *zs = nullptr;  // [n] sorted, wrapped
     double* qs = nullptr;                                // [n] sorted charges (per call)
+    // mesh binnings only: per-particle window coefficients (wave_bricks.cu, k_window_coef)
+    int* ws0[3] = {nullptr, nullptr, nullptr};      // first support mesh index per dimension
+    double* we0[3] = {nullptr, nullptr, nullptr};   // exp(-aw u0^2)
+    double* we1[3] = {nullptr, nullptr, nullptr};   // exp(-2 aw u0)
 };
 
 // real-space kernel constants (eq. 20/21)
@@ -175,14 +179,14 @@ int real_csr_build(pce_ctx* c, const Bins& b);
 int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s);
 
 // wave.cu
-int wave_spread(pce_ctx* c, const Bins& b);
 int wave_fft_scale_ifft(pce_ctx* c);
-int wave_gather(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
 
-// wave_tiles.cu
-int wave_tiles_init(pce_ctx* c);
-int wave_spread_tiles(pce_ctx* c, const Bins& b);
-int wave_gather_tiles(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+// wave_bricks.cu
+int wave_bricks_init(pce_ctx* c);
+int wave_coef_alloc(pce_ctx* c, Bins& b);
+int wave_window_coef(pce_ctx* c, const Bins& b);
+int wave_spread_bricks(pce_ctx* c, const Bins& b);
+int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
 
 // krylov.cu
 int bodies_setup(pce_ctx* c);

@@ -1,0 +1,518 @@
+// wave_bricks.cu -- output-stationary Gaussian spreading (eq. 25) and
+// brick-stationary Gaussian gather (eq. 27) for sm_100a.
+//
+// The paper spreads with one block of P^3 threads per particle and global atomics
+// (PAPER.md:263).  Here the mesh is cut into 8^3 bricks and ONE WARP owns one brick: lane l
+// holds the 4x4 (x,y) patch at (x0,y0) = (4(l&1), 4((l>>1)&1)), z = l>>2 in 16 fp64
+// REGISTERS.  Warps never synchronise with each other (no __syncthreads in the kernels):
+//   1. particles are binned by 8-point mesh bin (counting sort, cells.cu); the warp
+//      enumerates the <= 96 contiguous runs of the sorted particle list whose bins can hold
+//      a support that meets the brick, and walks them as one flat candidate list;
+//   2. test: one candidate per lane (3 int loads: the first support index per dimension),
+//      ballot, hits appended to a per-warp queue in shared memory;
+//   3. every 32 hits: lane l computes the 3x8 brick-local window weights of hit l from the
+//      per-particle coefficients of k_window_coef,
+//          exp(-aw (u0 + r)^2) = e0 * e1^r * G[r],   e0 = exp(-aw u0^2), e1 = exp(-2 aw u0)
+//      (no exp in these kernels), into a conflict-free padded table;
+//   4. accumulate: per hit every lane issues 5 shared-memory loads, 4 DMUL and 16 DFMA.
+// Spread writes every mesh point exactly once (no atomics, no memset, deterministic).
+// Gather keeps the brick of H~ in registers, reduces the 32 lane partials of 8 hits (4 with
+// the field) at a time by a transposing butterfly and issues one global fp64 atomicAdd per
+// hit and quantity.  The window is the truncated Gaussian of eq. 25 on exactly the P^3
+// nearest mesh points (reading A5), identical in both passes, so the mesh operator stays
+// symmetric.
+#include "pce_internal.h"
+
+constexpr int BR = 8;          // brick edge in mesh points
+constexpr int BWARPS = 4;      // warps (bricks) per CTA
+constexpr int MAXPIECE = 96;   // runs of candidates per brick: <= 6 x 6 rows x 2 wrap pieces (P <= 32)
+constexpr int STRIDE_PSI = 26; // doubles per hit in the weight table: 3 x 8 + 2 pad (13 x 16 B: conflict-free rows)
+constexpr int STRIDE_FLD = 50; // with the field: 3 x (8 w + 8 w u) + 2 pad (25 x 16 B)
+
+struct WinCoefPtrs {
+    const int* s0[3];
+    const double* e0[3];
+    const double* e1[3];
+};
+
+template <int STRIDE>
+struct alignas(16) WarpSmem {
+    double wt[32 * STRIDE];
+    int qidx[64];
+    int p_start[MAXPIECE];
+    int p_prefix[MAXPIECE + 1];
+};
+
+__device__ __forceinline__ int wrap_once(int d, int n) { if (d < 0) d += n; if (d >= n) d -= n; return d; }
+
+// bins (of BR mesh points) that can hold a particle whose support meets [b0, b0 + bw): the particle's
+// mesh cell i0 = floor(x/h) lies in [b0 - P/2, b0 + bw + P/2 - 2] (mod ng).  Up to two runs of bins.
+__device__ __forceinline__ int dim_bin_ranges(int b0, int bw, int P, int ng, int nc, int lo[2], int hi[2])
+{
+    const int a = b0 - P / 2, b = b0 + bw + P / 2 - 2;
+    if (b - a + 1 >= ng) { lo[0] = 0; hi[0] = nc - 1; return 1; }
+    const int aw = wrap_once(a, ng), bwp = wrap_once(b, ng);
+    if (aw <= bwp) { lo[0] = aw / BR; hi[0] = bwp / BR; return 1; }
+    if (bwp / BR >= aw / BR) { lo[0] = 0; hi[0] = nc - 1; return 1; }
+    lo[0] = 0; hi[0] = bwp / BR; lo[1] = aw / BR; hi[1] = nc - 1;
+    return 2;
+}
+
+struct Brick {
+    int b0[3], bw[3];
+    int npiece, M;
+};
+
+// brick of this warp and its candidate runs (p_start / p_prefix in the warp's shared memory)
+template <int STRIDE>
+__device__ __forceinline__ bool brick_setup(const WaveConst& wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start,
+                                            WarpSmem<STRIDE>& s, Brick& br, int lane, int brick_id)
+{
+    if (brick_id >= nbx * nby * nbz) return false;
+    const int nb[3] = {nbx, nby, nbz};
+    int t = brick_id;
+    const int bx = t % nbx; t /= nbx;
+    const int by = t % nby, bz = t / nby;
+    br.b0[0] = bx * BR; br.b0[1] = by * BR; br.b0[2] = bz * BR;
+    int lo[3][2], hi[3][2], nr[3], cnt[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        br.bw[d] = min(BR, wc.Ng[d] - br.b0[d]);
+        nr[d] = dim_bin_ranges(br.b0[d], br.bw[d], wc.P, wc.Ng[d], nb[d], lo[d], hi[d]);
+        cnt[d] = hi[d][0] - lo[d][0] + 1 + (nr[d] == 2 ? hi[d][1] - lo[d][1] + 1 : 0);  // bins in y, z
+    }
+    // pieces: (z bin, y bin, x run)
+    const int npiece = cnt[2] * cnt[1] * nr[0];
+    br.npiece = npiece;  // <= MAXPIECE by construction (P <= 32)
+    int carry = 0;
+    for (int base = 0; base < npiece; base += 32) {
+        const int k = base + lane;
+        int len = 0, start = 0;
+        if (k < npiece) {
+            const int xr = k % nr[0];
+            int r = k / nr[0];
+            const int yi = r % cnt[1], zi = r / cnt[1];
+            const int n0y = hi[1][0] - lo[1][0] + 1, n0z = hi[2][0] - lo[2][0] + 1;
+            const int yb = (yi < n0y) ? lo[1][0] + yi : lo[1][1] + (yi - n0y);
+            const int zb = (zi < n0z) ? lo[2][0] + zi : lo[2][1] + (zi - n0z);
+            const int row = (zb * nby + yb) * nbx;
+            start = cell_start[row + lo[0][xr]];
+            len = cell_start[row + hi[0][xr] + 1] - start;
+        }
+        int incl = len;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += v;
+        }
+        if (k < npiece) { s.p_start[k] = start; s.p_prefix[k] = carry + incl - len; }
+        carry += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) s.p_prefix[npiece] = carry;
+    br.M = carry;
+    __syncwarp();
+    return true;
+}
+
+// flat candidate index -> sorted particle slot
+template <int STRIDE>
+__device__ __forceinline__ int candidate_slot(const WarpSmem<STRIDE>& s, int npiece, int c)
+{
+    int lo = 0, hi = npiece;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (c >= s.p_prefix[mid]) lo = mid; else hi = mid;
+    }
+    return s.p_start[lo] + (c - s.p_prefix[lo]);
+}
+
+__device__ __forceinline__ bool support_meets_brick(const WaveConst& wc, const Brick& br, const WinCoefPtrs& wp, int pi)
+{
+    bool hit = true;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int ng = wc.Ng[d];
+        const int dsl = wrap_once(br.b0[d] - wp.s0[d][pi], ng);  // brick origin - first support index, mod ng
+        hit = hit && (dsl < wc.P || dsl + br.bw[d] > ng);
+    }
+    return hit;
+}
+
+// the 8 brick-local window weights of one particle in one dimension (0 outside the support)
+template <bool FIELD>
+__device__ __forceinline__ void brick_weights(const WaveConst& wc, const double* __restrict__ Gs, int b0, int ng, int s0, double e0,
+                                              double e1, double u0, double scale, double* __restrict__ w)
+{
+    const int P = wc.P;
+    const int dsl = wrap_once(b0 - s0, ng);
+    double pw = 0.0;
+    if (dsl < P) {  // e0 e1^dsl
+        double r = e0, b = e1;
+        int n = dsl;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            if (n & 1) r *= b;
+            b *= b;
+            n >>= 1;
+        }
+        pw = r;
+    }
+    int r = dsl;
+    double v[BR], vu[BR];
+#pragma unroll
+    for (int j = 0; j < BR; ++j) {
+        const bool in = r < P;
+        const double g = Gs[in ? r : 0];
+        v[j] = in ? pw * g * scale : 0.0;
+        if (FIELD) vu[j] = v[j] * (u0 + (double)r);
+        pw *= e1;
+        ++r;
+        if (r == ng) { r = 0; pw = e0; }
+    }
+#pragma unroll
+    for (int j = 0; j < BR; j += 2) *reinterpret_cast<double2*>(w + j) = make_double2(v[j], v[j + 1]);
+    if (FIELD) {
+#pragma unroll
+        for (int j = 0; j < BR; j += 2) *reinterpret_cast<double2*>(w + BR + j) = make_double2(vu[j], vu[j + 1]);
+    }
+}
+
+// hits appended by the test phase; process() consumes the first min(nq, 32)
+#define BRICK_WALK(PROCESS)                                                                        \
+    int nq = 0;                                                                                    \
+    for (int cb = 0; cb < br.M; cb += 32) {                                                        \
+        const int c = cb + lane;                                                                   \
+        bool hit = false;                                                                          \
+        int pi = 0;                                                                                \
+        if (c < br.M) {                                                                            \
+            pi = candidate_slot(s, br.npiece, c);                                                  \
+            hit = support_meets_brick(wc, br, wp, pi);                                             \
+        }                                                                                          \
+        const unsigned m = __ballot_sync(0xffffffffu, hit);                                        \
+        if (hit) s.qidx[nq + __popc(m & ((1u << lane) - 1u))] = pi;                                \
+        nq += __popc(m);                                                                           \
+        __syncwarp();                                                                              \
+        if (nq >= 32) {                                                                            \
+            PROCESS(32);                                                                           \
+            const int rest = nq - 32;                                                              \
+            const int v = (lane < rest) ? s.qidx[32 + lane] : 0;                                   \
+            __syncwarp();                                                                          \
+            if (lane < rest) s.qidx[lane] = v;                                                     \
+            nq = rest;                                                                             \
+            __syncwarp();                                                                          \
+        }                                                                                          \
+    }                                                                                              \
+    if (nq > 0) { PROCESS(nq); }
+
+// ---------------------------------------------------------------- window coefficients (once per position update)
+__global__ void __launch_bounds__(256)
+k_window_coef(int n, WaveConst wc, const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+              int* __restrict__ s0x, int* __restrict__ s0y, int* __restrict__ s0z, double* __restrict__ e0x, double* __restrict__ e0y,
+              double* __restrict__ e0z, double* __restrict__ e1x, double* __restrict__ e1y, double* __restrict__ e1z)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double pos[3] = {xs[i], ys[i], zs[i]};
+    int* so[3] = {s0x, s0y, s0z};
+    double* a0[3] = {e0x, e0y, e0z};
+    double* a1[3] = {e1x, e1y, e1z};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double xd = pos[d] * wc.inv_h[d];
+        const int i0 = min((int)xd, wc.Ng[d] - 1);
+        const int s0 = i0 - wc.P / 2 + 1;  // first support index (reading A5, even P); may be negative
+        const double u0 = (double)s0 - xd; // in (-P/2, -P/2 + 1]
+        so[d][i] = s0;
+        a0[d][i] = exp(-wc.aw * u0 * u0);
+        a1[d][i] = exp(-2.0 * wc.aw * u0);
+    }
+}
+
+// ---------------------------------------------------------------- spread
+__global__ void __launch_bounds__(BWARPS * 32)
+k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
+                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* Gs = reinterpret_cast<double*>(smem_raw);
+    WarpSmem<STRIDE_PSI>* sm = reinterpret_cast<WarpSmem<STRIDE_PSI>*>(smem_raw + 32 * sizeof(double));
+    if (threadIdx.x < 32) Gs[threadIdx.x] = wc.G[threadIdx.x];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpSmem<STRIDE_PSI>& s = sm[warp];
+    Brick br;
+    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, blockIdx.x * BWARPS + warp)) return;
+    const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    double acc[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[j][i] = 0.0;
+
+#define SPREAD_PROCESS(NH)                                                                                              \
+    {                                                                                                                   \
+        const int nh = (NH);                                                                                            \
+        if (lane < nh) {                                                                                                \
+            const int p = s.qidx[lane];                                                                                 \
+            const double qv = qs[p];                                                                                    \
+            double* w = s.wt + lane * STRIDE_PSI;                                                                       \
+            _Pragma("unroll") for (int d = 0; d < 3; ++d)                                                               \
+                brick_weights<false>(wc, Gs, br.b0[d], wc.Ng[d], wp.s0[d][p], wp.e0[d][p], wp.e1[d][p], 0.0,            \
+                                     d == 2 ? qv : 1.0, w + BR * d);                                                    \
+        }                                                                                                               \
+        __syncwarp();                                                                                                   \
+        for (int slot = 0; slot < nh; ++slot) {                                                                         \
+            const double* w = s.wt + slot * STRIDE_PSI;                                                                 \
+            const double2 x01 = *reinterpret_cast<const double2*>(w + px);                                              \
+            const double2 x23 = *reinterpret_cast<const double2*>(w + px + 2);                                          \
+            const double2 y01 = *reinterpret_cast<const double2*>(w + BR + py);                                         \
+            const double2 y23 = *reinterpret_cast<const double2*>(w + BR + py + 2);                                     \
+            const double wzq = w[2 * BR + pz];                                                                          \
+            const double cy[4] = {wzq * y01.x, wzq * y01.y, wzq * y23.x, wzq * y23.y};                                  \
+            const double wx[4] = {x01.x, x01.y, x23.x, x23.y};                                                          \
+            _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                               \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) acc[j][i] = fma(cy[j], wx[i], acc[j][i]);                 \
+        }                                                                                                               \
+        __syncwarp();                                                                                                   \
+    }
+
+    BRICK_WALK(SPREAD_PROCESS)
+#undef SPREAD_PROCESS
+
+    const int gz = br.b0[2] + pz;
+    if (gz >= wc.Ng[2]) return;
+    const size_t Nx = wc.Ng[0], Ny = wc.Ng[1];
+    const int gx = br.b0[0] + px;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int gy = br.b0[1] + py + j;
+        if (gy >= wc.Ng[1]) break;
+        double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
+        if (vec_ok && gx + 3 < wc.Ng[0]) {
+            *reinterpret_cast<double2*>(row) = make_double2(acc[j][0], acc[j][1]);
+            *reinterpret_cast<double2*>(row + 2) = make_double2(acc[j][2], acc[j][3]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (gx + i < wc.Ng[0]) row[i] = acc[j][i];
+        }
+    }
+}
+
+// ---------------------------------------------------------------- gather
+// reduce NV values per lane across the warp; afterwards lanes with (lane & (32/NV - 1)) == 0 hold the warp
+// total of value number `id`
+template <int NV>
+__device__ __forceinline__ double transpose_reduce(double (&v)[NV], int lane, int& id)
+{
+    id = 0;
+    int x = 16;
+#pragma unroll
+    for (int half = NV / 2; half >= 1; half >>= 1) {
+        const bool up = (lane & x) != 0;
+#pragma unroll
+        for (int k = 0; k < half; ++k) {
+            const double send = up ? v[k] : v[k + half];
+            const double keep = up ? v[k + half] : v[k];
+            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, x);
+        }
+        if (up) id += half;
+        x >>= 1;
+    }
+    double r = v[0];
+    for (; x >= 1; x >>= 1) r += __shfl_xor_sync(0xffffffffu, r, x);
+    return r;
+}
+
+template <bool FIELD>
+__global__ void __launch_bounds__(BWARPS * 32)
+k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
+                const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                const double* __restrict__ grid, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
+                double* __restrict__ ez, int vec_ok)
+{
+    constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
+    constexpr int DW = FIELD ? 2 * BR : BR;  // doubles per dimension in the weight table
+    constexpr int G = FIELD ? 4 : 8;         // hits per butterfly
+    constexpr int NQ = FIELD ? 4 : 1;        // quantities per hit: psi (, Ex, Ey, Ez)
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* Gs = reinterpret_cast<double*>(smem_raw);
+    WarpSmem<STRIDE>* sm = reinterpret_cast<WarpSmem<STRIDE>*>(smem_raw + 32 * sizeof(double));
+    if (threadIdx.x < 32) Gs[threadIdx.x] = wc.G[threadIdx.x];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpSmem<STRIDE>& s = sm[warp];
+    Brick br;
+    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, blockIdx.x * BWARPS + warp)) return;
+    if (br.M == 0) return;
+    const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    // the lane's 4x4 patch of H~ in registers (0 outside the mesh)
+    double H[4][4];
+    {
+        const size_t Nx = wc.Ng[0], Ny = wc.Ng[1];
+        const int gz = br.b0[2] + pz, gx = br.b0[0] + px;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int gy = br.b0[1] + py + j;
+            const bool rowok = gz < wc.Ng[2] && gy < wc.Ng[1];
+            const double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
+            if (rowok && vec_ok && gx + 3 < wc.Ng[0]) {
+                const double2 a = *reinterpret_cast<const double2*>(row), b = *reinterpret_cast<const double2*>(row + 2);
+                H[j][0] = a.x; H[j][1] = a.y; H[j][2] = b.x; H[j][3] = b.y;
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) H[j][i] = (rowok && gx + i < wc.Ng[0]) ? row[i] : 0.0;
+            }
+        }
+    }
+
+#define GATHER_PROCESS(NH)                                                                                              \
+    {                                                                                                                   \
+        const int nh = (NH);                                                                                            \
+        if (lane < nh) {                                                                                                \
+            const int p = s.qidx[lane];                                                                                 \
+            double* w = s.wt + lane * STRIDE;                                                                           \
+            const double pos[3] = {FIELD ? xs[p] : 0.0, FIELD ? ys[p] : 0.0, FIELD ? zs[p] : 0.0};                      \
+            _Pragma("unroll") for (int d = 0; d < 3; ++d) {                                                             \
+                const int s0 = wp.s0[d][p];                                                                             \
+                const double u0 = FIELD ? (double)s0 - pos[d] * wc.inv_h[d] : 0.0;                                      \
+                brick_weights<FIELD>(wc, Gs, br.b0[d], wc.Ng[d], s0, wp.e0[d][p], wp.e1[d][p], u0, 1.0, w + DW * d);    \
+            }                                                                                                           \
+        }                                                                                                               \
+        __syncwarp();                                                                                                   \
+        for (int sb = 0; sb < nh; sb += G) {                                                                            \
+            double v[NQ * G];                                                                                           \
+            _Pragma("unroll") for (int g = 0; g < G; ++g) {                                                             \
+                if (sb + g < nh) {                                                                                      \
+                    const double* w = s.wt + (sb + g) * STRIDE;                                                         \
+                    const double2 x01 = *reinterpret_cast<const double2*>(w + px);                                      \
+                    const double2 x23 = *reinterpret_cast<const double2*>(w + px + 2);                                  \
+                    const double2 y01 = *reinterpret_cast<const double2*>(w + DW + py);                                 \
+                    const double2 y23 = *reinterpret_cast<const double2*>(w + DW + py + 2);                             \
+                    const double wz = w[2 * DW + pz];                                                                   \
+                    const double wx[4] = {x01.x, x01.y, x23.x, x23.y};                                                  \
+                    const double wy[4] = {y01.x, y01.y, y23.x, y23.y};                                                  \
+                    double t0[4];                                                                                       \
+                    _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                       \
+                        t0[j] = fma(H[j][3], wx[3], fma(H[j][2], wx[2], fma(H[j][1], wx[1], H[j][0] * wx[0])));         \
+                    const double s0 = fma(wy[3], t0[3], fma(wy[2], t0[2], fma(wy[1], t0[1], wy[0] * t0[0])));           \
+                    if (!FIELD) {                                                                                       \
+                        v[g] = wz * s0;                                                                                 \
+                    } else {                                                                                            \
+                        const double2 xu01 = *reinterpret_cast<const double2*>(w + BR + px);                            \
+                        const double2 xu23 = *reinterpret_cast<const double2*>(w + BR + px + 2);                        \
+                        const double2 yu01 = *reinterpret_cast<const double2*>(w + DW + BR + py);                       \
+                        const double2 yu23 = *reinterpret_cast<const double2*>(w + DW + BR + py + 2);                   \
+                        const double wzu = w[2 * DW + BR + pz];                                                         \
+                        const double wxu[4] = {xu01.x, xu01.y, xu23.x, xu23.y};                                         \
+                        const double wyu[4] = {yu01.x, yu01.y, yu23.x, yu23.y};                                         \
+                        double t1[4];                                                                                   \
+                        _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                   \
+                            t1[j] = fma(H[j][3], wxu[3], fma(H[j][2], wxu[2], fma(H[j][1], wxu[1], H[j][0] * wxu[0]))); \
+                        const double sx = fma(wy[3], t1[3], fma(wy[2], t1[2], fma(wy[1], t1[1], wy[0] * t1[0])));       \
+                        const double sy = fma(wyu[3], t0[3], fma(wyu[2], t0[2], fma(wyu[1], t0[1], wyu[0] * t0[0])));   \
+                        v[NQ * g + 0] = wz * s0;                                                                        \
+                        v[NQ * g + 1] = wz * sx;                                                                        \
+                        v[NQ * g + 2] = wz * sy;                                                                        \
+                        v[NQ * g + 3] = wzu * s0;                                                                       \
+                    }                                                                                                   \
+                } else {                                                                                                \
+                    _Pragma("unroll") for (int k = 0; k < NQ; ++k) v[NQ * g + k] = 0.0;                                 \
+                }                                                                                                       \
+            }                                                                                                           \
+            int id;                                                                                                     \
+            const double r = transpose_reduce<NQ * G>(v, lane, id);                                                     \
+            const int g = id / NQ, qn = id - g * NQ;                                                                    \
+            if ((lane & (32 / (NQ * G) - 1)) == 0 && sb + g < nh) {                                                     \
+                const int p = s.qidx[sb + g];                                                                           \
+                if (qn == 0) atomicAdd(&psi[p], r);                                                                     \
+                else if (qn == 1) atomicAdd(&ex[p], -wc.grad_fac[0] * r); /* E = -grad_a, dW/dx_a = +grad_fac u W */    \
+                else if (qn == 2) atomicAdd(&ey[p], -wc.grad_fac[1] * r);                                               \
+                else atomicAdd(&ez[p], -wc.grad_fac[2] * r);                                                            \
+            }                                                                                                           \
+        }                                                                                                               \
+        __syncwarp();                                                                                                   \
+    }
+
+    BRICK_WALK(GATHER_PROCESS)
+#undef GATHER_PROCESS
+}
+
+// ---------------------------------------------------------------- host
+static size_t smem_bytes(bool field)
+{
+    return 32 * sizeof(double) + BWARPS * (field ? sizeof(WarpSmem<STRIDE_FLD>) : sizeof(WarpSmem<STRIDE_PSI>));
+}
+
+int wave_bricks_init(pce_ctx* c)
+{
+    PCE_CUDA(c, cudaFuncSetAttribute(k_spread_bricks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(false)));
+    PCE_CUDA(c, cudaFuncSetAttribute(k_gather_bricks<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(false)));
+    PCE_CUDA(c, cudaFuncSetAttribute(k_gather_bricks<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(true)));
+    return PCE_OK;
+}
+
+int wave_coef_alloc(pce_ctx* c, Bins& b)
+{
+    const size_t n = (size_t)(b.n > 0 ? b.n : 1);
+    for (int d = 0; d < 3; ++d) {
+        PCE_CUDA(c, cudaMalloc(&b.ws0[d], n * sizeof(int)));
+        PCE_CUDA(c, cudaMalloc(&b.we0[d], n * sizeof(double)));
+        PCE_CUDA(c, cudaMalloc(&b.we1[d], n * sizeof(double)));
+    }
+    c->bytes += (long long)(n * 60);
+    return PCE_OK;
+}
+
+// per-particle window coefficients of a mesh binning (after bins_build)
+int wave_window_coef(pce_ctx* c, const Bins& b)
+{
+    if (b.n == 0) return PCE_OK;
+    k_window_coef<<<cdiv(b.n, 256), 256, 0, c->st>>>(b.n, c->wk, b.xs, b.ys, b.zs, b.ws0[0], b.ws0[1], b.ws0[2], b.we0[0], b.we0[1],
+                                                     b.we0[2], b.we1[0], b.we1[1], b.we1[2]);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+static WinCoefPtrs coef_ptrs(const Bins& b)
+{
+    WinCoefPtrs p;
+    for (int d = 0; d < 3; ++d) { p.s0[d] = b.ws0[d]; p.e0[d] = b.we0[d]; p.e1[d] = b.we1[d]; }
+    return p;
+}
+
+int wave_spread_bricks(pce_ctx* c, const Bins& b)
+{
+    PassTimer t(c, PASS_SPREAD);
+    const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
+    k_spread_bricks<<<cdiv(b.ncell, BWARPS), BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
+                                                                                     coef_ptrs(b), b.qs, c->grid, vec_ok);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s)
+{
+    if (b.n == 0) return PCE_OK;
+    PassTimer t(c, PASS_GATHER);
+    const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
+    const int blocks = cdiv(b.ncell, BWARPS);
+    PCE_CUDA(c, cudaMemsetAsync(psi_s, 0, (size_t)b.n * sizeof(double), c->st));
+    if (field) {
+        PCE_CUDA(c, cudaMemsetAsync(ex_s, 0, (size_t)b.n * sizeof(double), c->st));
+        PCE_CUDA(c, cudaMemsetAsync(ey_s, 0, (size_t)b.n * sizeof(double), c->st));
+        PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
+        k_gather_bricks<true><<<blocks, BWARPS * 32, smem_bytes(true), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
+                                                                               coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, ex_s, ey_s,
+                                                                               ez_s, vec_ok);
+    } else {
+        k_gather_bricks<false><<<blocks, BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
+                                                                                 coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, nullptr,
+                                                                                 nullptr, nullptr, vec_ok);
+    }
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
