@@ -128,13 +128,18 @@ int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double*
 // ---------------------------------------------------------------- binning
 __global__ void k_cell_count(int n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                              int ncx, int ncy, int ncz, double sx, double sy, double sz, int mx, int my, int mz, int dvx, int dvy,
-                             int dvz, int* __restrict__ cell_of, int* __restrict__ count)
+                             int dvz, int shx, int shy, int shz, int* __restrict__ cell_of, int* __restrict__ count)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    int cx = min(min((int)(x[i] * sx), mx) / dvx, ncx - 1);
-    int cy = min(min((int)(y[i] * sy), my) / dvy, ncy - 1);
-    int cz = min(min((int)(z[i] * sz), mz) / dvz, ncz - 1);
+    // index along each dimension, cyclically shifted by sh (mesh bins only), then divided into bins
+    int ix = min((int)(x[i] * sx), mx) + shx, iy = min((int)(y[i] * sy), my) + shy, iz = min((int)(z[i] * sz), mz) + shz;
+    if (ix > mx) ix -= mx + 1;
+    if (iy > my) iy -= my + 1;
+    if (iz > mz) iz -= mz + 1;
+    int cx = min(ix / dvx, ncx - 1);
+    int cy = min(iy / dvy, ncy - 1);
+    int cz = min(iz / dvz, ncz - 1);
     const int cidx = (cz * ncy + cy) * ncx + cx;
     cell_of[i] = cidx;
     atomicAdd(&count[cidx], 1);
@@ -213,7 +218,10 @@ int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile)
     int rc = bins_alloc(c, b, n, nc, range);
     if (rc) return rc;
     // the same 1/h the mesh kernels use, so that floor(x/h) agrees bit for bit
-    for (int d = 0; d < 3; ++d) { b.scale[d] = c->wk.inv_h[d]; b.imax[d] = c->p.Ng[d] - 1; b.div[d] = tile; }
+    // bins are shifted by P/2 mod tile so that the mesh cells whose support meets a brick span the fewest bins
+    for (int d = 0; d < 3; ++d) {
+        b.scale[d] = c->wk.inv_h[d]; b.imax[d] = c->p.Ng[d] - 1; b.div[d] = tile; b.shift[d] = (c->p.P / 2) % tile;
+    }
     return PCE_OK;
 }
 
@@ -221,7 +229,7 @@ void bins_free(Bins& b)
 {
     cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp); cudaFree(b.inv);
     cudaFree(b.xs); cudaFree(b.ys); cudaFree(b.zs); cudaFree(b.qs);
-    for (int d = 0; d < 3; ++d) { cudaFree(b.ws0[d]); cudaFree(b.we0[d]); cudaFree(b.we1[d]); }
+    cudaFree(b.ws0); cudaFree(b.wcf);
     b = Bins();
 }
 
@@ -243,7 +251,8 @@ int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const doub
         PCE_CUDA(c, cudaMemsetAsync(b.cell_start, 0, ((size_t)b.ncell + 1) * sizeof(int), c->st));
         PCE_CUDA(c, cudaMemsetAsync(b.cell_fill, 0, ((size_t)b.ncell + 1) * sizeof(int), c->st));
         k_cell_count<<<cdiv(n, 256), 256, 0, c->st>>>(n, x, y, z, b.nc[0], b.nc[1], b.nc[2], b.scale[0], b.scale[1], b.scale[2],
-                                                      b.imax[0], b.imax[1], b.imax[2], b.div[0], b.div[1], b.div[2], b.cell_of,
+                                                      b.imax[0], b.imax[1], b.imax[2], b.div[0], b.div[1], b.div[2], b.shift[0],
+                                                      b.shift[1], b.shift[2], b.cell_of,
                                                       b.cell_start);
         c->launches++;
         int rc = exclusive_scan(c, b.cell_start, b.ncell + 1);

@@ -23,10 +23,11 @@ struct Bins {
     int ncell = 1;
     int range[3] = {1, 1, 1};  // stencil half width: 1 (cells) or image count
     double L[3];
-    // cell index per dimension = min(min((int)(x * scale), imax) / div, nc - 1):
-    //   real-space cells: scale = nc/L, div = 1;  mesh tiles: scale = 1/h, imax = Ng-1, div = tile edge
+    // cell index per dimension = min(((min((int)(x * scale), imax) + shift) mod (imax + 1)) / div, nc - 1):
+    //   real-space cells: scale = nc/L, div = 1, shift = 0;
+    //   mesh bins: scale = 1/h, imax = Ng-1, div = brick edge, shift = P/2 mod brick edge
     double scale[3] = {1, 1, 1};
-    int imax[3] = {0, 0, 0}, div[3] = {1, 1, 1};
+    int imax[3] = {0, 0, 0}, div[3] = {1, 1, 1}, shift[3] = {0, 0, 0};
     int* inv = nullptr;         // [n] index in the subset -> sorted slot
     int* cell_of = nullptr;     // [n]
     int* cell_start = nullptr;  // [ncell+1]
@@ -36,9 +37,8 @@ struct Bins {
     double *xs = nullptr, *ys = nullptr, *zs = nullptr;  // [n] sorted, wrapped
     double* qs = nullptr;                                // [n] sorted charges (per call)
     // mesh binnings only: per-particle window coefficients (wave_bricks.cu, k_window_coef)
-    int* ws0[3] = {nullptr, nullptr, nullptr};      // first support mesh index per dimension
-    double* we0[3] = {nullptr, nullptr, nullptr};   // exp(-aw u0^2)
-    double* we1[3] = {nullptr, nullptr, nullptr};   // exp(-2 aw u0)
+    int4* ws0 = nullptr;      // [n] first support mesh index per dimension (x, y, z, unused)
+    double4* wcf = nullptr;   // [3 n] per particle and dimension: (c0, e1, e8, 1/e8), see wave_bricks.cu
 };
 
 // real-space kernel constants (eq. 20/21)

@@ -4,23 +4,28 @@
 // The paper spreads with one block of P^3 threads per particle and global atomics
 // (PAPER.md:263).  Here the mesh is cut into 8^3 bricks and ONE WARP owns one brick: lane l
 // holds the 4x4 (x,y) patch at (x0,y0) = (4(l&1), 4((l>>1)&1)), z = l>>2 in 16 fp64
-// REGISTERS.  Warps never synchronise with each other (no __syncthreads in the kernels):
-//   1. particles are binned by 8-point mesh bin (counting sort, cells.cu); the warp
-//      enumerates the <= 96 contiguous runs of the sorted particle list whose bins can hold
-//      a support that meets the brick, and walks them as one flat candidate list;
-//   2. test: one candidate per lane (3 int loads: the first support index per dimension),
-//      ballot, hits appended to a per-warp queue in shared memory;
-//   3. every 32 hits: lane l computes the 3x8 brick-local window weights of hit l from the
-//      per-particle coefficients of k_window_coef,
-//          exp(-aw (u0 + r)^2) = e0 * e1^r * G[r],   e0 = exp(-aw u0^2), e1 = exp(-2 aw u0)
-//      (no exp in these kernels), into a conflict-free padded table;
+// REGISTERS.  Warps never synchronise with each other (one __syncthreads after the table
+// load, none afterwards):
+//   1. particles are binned by 8-point mesh bin (counting sort, cells.cu; bins shifted by
+//      P/2 mod 8 so that the cells whose support meets a brick span ceil((P+7)/8) bins per
+//      dimension); the warp enumerates the contiguous runs of the sorted particle list in
+//      those bins and walks them as one flat candidate list;
+//   2. test: one candidate per lane (one 16-byte load: the first support index per
+//      dimension), ballot, hits appended to a per-warp queue in shared memory;
+//   3. every 32 hits: lane l computes the 3x8 brick-local window weights of hit l.  With
+//      u = u0 + r the offset of support point r from the particle (mesh units),
+//          W(r) = exp(-aw u^2),  W(r+1) = W(r) t(r),  t(r+1) = t(r) exp(-2 aw),
+//      started from per-particle coefficients of k_window_coef (phi = -s0 mod 8,
+//      e1 = exp(-2 aw u0), c0 = exp(-aw u0^2) e1^phi, e8 = e1^8):
+//      W(phi + 8m) = c0 e8^m exp(-aw (phi + 8m)^2), t(r) = e1 exp(-aw (2r + 1)); no exp here;
 //   4. accumulate: per hit every lane issues 5 shared-memory loads, 4 DMUL and 16 DFMA.
 // Spread writes every mesh point exactly once (no atomics, no memset, deterministic).
 // Gather keeps the brick of H~ in registers, reduces the 32 lane partials of 8 hits (4 with
 // the field) at a time by a transposing butterfly and issues one global fp64 atomicAdd per
 // hit and quantity.  The window is the truncated Gaussian of eq. 25 on exactly the P^3
 // nearest mesh points (reading A5), identical in both passes, so the mesh operator stays
-// symmetric.
+// symmetric.  Grids with Ng % 8 != 0 or Ng - P < 8 take a generic weight routine (direct
+// exp, wrap-aware); everything else is shared.
 #include "pce_internal.h"
 
 constexpr int BR = 8;          // brick edge in mesh points
@@ -28,11 +33,11 @@ constexpr int BWARPS = 4;      // warps (bricks) per CTA
 constexpr int MAXPIECE = 96;   // runs of candidates per brick: <= 6 x 6 rows x 2 wrap pieces (P <= 32)
 constexpr int STRIDE_PSI = 26; // doubles per hit in the weight table: 3 x 8 + 2 pad (13 x 16 B: conflict-free rows)
 constexpr int STRIDE_FLD = 50; // with the field: 3 x (8 w + 8 w u) + 2 pad (25 x 16 B)
+constexpr int NTAB = 48 + 48;  // Gt[r + 8] = exp(-aw r^2), Ht[r + 8] = exp(-aw (2r + 1)), r = -8..39
 
 struct WinCoefPtrs {
-    const int* s0[3];
-    const double* e0[3];
-    const double* e1[3];
+    const int4* s0;       // [n]
+    const double4* cf;    // [3 n]: (c0, e1, e8, 1/e8) of particle p, dimension d at 3 p + d
 };
 
 template <int STRIDE>
@@ -40,18 +45,19 @@ struct alignas(16) WarpSmem {
     double wt[32 * STRIDE];
     int qidx[64];
     int p_start[MAXPIECE];
-    int p_prefix[MAXPIECE + 1];
+    int p_prefix[MAXPIECE + 4];
 };
 
 __device__ __forceinline__ int wrap_once(int d, int n) { if (d < 0) d += n; if (d >= n) d -= n; return d; }
 
-// bins (of BR mesh points) that can hold a particle whose support meets [b0, b0 + bw): the particle's
-// mesh cell i0 = floor(x/h) lies in [b0 - P/2, b0 + bw + P/2 - 2] (mod ng).  Up to two runs of bins.
+// bins (of BR shifted mesh cells) that can hold a particle whose support meets [b0, b0 + bw): the particle's
+// mesh cell i0 = floor(x/h) lies in [b0 - P/2, b0 + bw + P/2 - 2] (mod ng); bins are over (i0 + shift) mod ng.
 __device__ __forceinline__ int dim_bin_ranges(int b0, int bw, int P, int ng, int nc, int lo[2], int hi[2])
 {
-    const int a = b0 - P / 2, b = b0 + bw + P / 2 - 2;
+    const int shift = (P / 2) % BR;
+    const int a = b0 - P / 2 + shift, b = b0 + bw + P / 2 - 2 + shift;
     if (b - a + 1 >= ng) { lo[0] = 0; hi[0] = nc - 1; return 1; }
-    const int aw = wrap_once(a, ng), bwp = wrap_once(b, ng);
+    const int aw = wrap_once(wrap_once(a, ng), ng), bwp = wrap_once(wrap_once(b, ng), ng);
     if (aw <= bwp) { lo[0] = aw / BR; hi[0] = bwp / BR; return 1; }
     if (bwp / BR >= aw / BR) { lo[0] = 0; hi[0] = nc - 1; return 1; }
     lo[0] = 0; hi[0] = bwp / BR; lo[1] = aw / BR; hi[1] = nc - 1;
@@ -69,35 +75,34 @@ __device__ __forceinline__ bool brick_setup(const WaveConst& wc, int nbx, int nb
                                             WarpSmem<STRIDE>& s, Brick& br, int lane, int brick_id)
 {
     if (brick_id >= nbx * nby * nbz) return false;
-    const int nb[3] = {nbx, nby, nbz};
     int t = brick_id;
     const int bx = t % nbx; t /= nbx;
     const int by = t % nby, bz = t / nby;
     br.b0[0] = bx * BR; br.b0[1] = by * BR; br.b0[2] = bz * BR;
-    int lo[3][2], hi[3][2], nr[3], cnt[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        br.bw[d] = min(BR, wc.Ng[d] - br.b0[d]);
-        nr[d] = dim_bin_ranges(br.b0[d], br.bw[d], wc.P, wc.Ng[d], nb[d], lo[d], hi[d]);
-        cnt[d] = hi[d][0] - lo[d][0] + 1 + (nr[d] == 2 ? hi[d][1] - lo[d][1] + 1 : 0);  // bins in y, z
-    }
+    br.bw[0] = min(BR, wc.Ng[0] - br.b0[0]); br.bw[1] = min(BR, wc.Ng[1] - br.b0[1]); br.bw[2] = min(BR, wc.Ng[2] - br.b0[2]);
+    int lox[2], hix[2], loy[2], hiy[2], loz[2], hiz[2];
+    const int nrx = dim_bin_ranges(br.b0[0], br.bw[0], wc.P, wc.Ng[0], nbx, lox, hix);
+    const int nry = dim_bin_ranges(br.b0[1], br.bw[1], wc.P, wc.Ng[1], nby, loy, hiy);
+    const int nrz = dim_bin_ranges(br.b0[2], br.bw[2], wc.P, wc.Ng[2], nbz, loz, hiz);
+    const int n0y = hiy[0] - loy[0] + 1, n0z = hiz[0] - loz[0] + 1;
+    const int cnty = n0y + (nry == 2 ? hiy[1] - loy[1] + 1 : 0);  // bins in y
+    const int cntz = n0z + (nrz == 2 ? hiz[1] - loz[1] + 1 : 0);  // bins in z
     // pieces: (z bin, y bin, x run)
-    const int npiece = cnt[2] * cnt[1] * nr[0];
+    const int npiece = cntz * cnty * nrx;
     br.npiece = npiece;  // <= MAXPIECE by construction (P <= 32)
     int carry = 0;
     for (int base = 0; base < npiece; base += 32) {
         const int k = base + lane;
         int len = 0, start = 0;
         if (k < npiece) {
-            const int xr = k % nr[0];
-            int r = k / nr[0];
-            const int yi = r % cnt[1], zi = r / cnt[1];
-            const int n0y = hi[1][0] - lo[1][0] + 1, n0z = hi[2][0] - lo[2][0] + 1;
-            const int yb = (yi < n0y) ? lo[1][0] + yi : lo[1][1] + (yi - n0y);
-            const int zb = (zi < n0z) ? lo[2][0] + zi : lo[2][1] + (zi - n0z);
+            const int xr = (nrx == 2) ? (k & 1) : 0;
+            const int r = (nrx == 2) ? (k >> 1) : k;
+            const int zi = r / cnty, yi = r - zi * cnty;
+            const int yb = (yi < n0y) ? loy[0] + yi : loy[1] + (yi - n0y);
+            const int zb = (zi < n0z) ? loz[0] + zi : loz[1] + (zi - n0z);
             const int row = (zb * nby + yb) * nbx;
-            start = cell_start[row + lo[0][xr]];
-            len = cell_start[row + hi[0][xr] + 1] - start;
+            start = cell_start[row + (xr ? lox[1] : lox[0])];
+            len = cell_start[row + (xr ? hix[1] : hix[0]) + 1] - start;
         }
         int incl = len;
 #pragma unroll
@@ -114,60 +119,56 @@ __device__ __forceinline__ bool brick_setup(const WaveConst& wc, int nbx, int nb
     return true;
 }
 
-// flat candidate index -> sorted particle slot
-template <int STRIDE>
-__device__ __forceinline__ int candidate_slot(const WarpSmem<STRIDE>& s, int npiece, int c)
+__device__ __forceinline__ bool support_meets_brick(const WaveConst& wc, const Brick& br, const int4 s0)
 {
-    int lo = 0, hi = npiece;
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (c >= s.p_prefix[mid]) lo = mid; else hi = mid;
-    }
-    return s.p_start[lo] + (c - s.p_prefix[lo]);
-}
-
-__device__ __forceinline__ bool support_meets_brick(const WaveConst& wc, const Brick& br, const WinCoefPtrs& wp, int pi)
-{
+    const int sv[3] = {s0.x, s0.y, s0.z};
     bool hit = true;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const int ng = wc.Ng[d];
-        const int dsl = wrap_once(br.b0[d] - wp.s0[d][pi], ng);  // brick origin - first support index, mod ng
+        const int dsl = wrap_once(br.b0[d] - sv[d], ng);  // brick origin - first support index, mod ng
         hit = hit && (dsl < wc.P || dsl + br.bw[d] > ng);
     }
     return hit;
 }
 
-// the 8 brick-local window weights of one particle in one dimension (0 outside the support)
+// the 8 brick-local window weights of one particle in one dimension (0 outside the support), and with FIELD the
+// weights times u = (mesh index - x/h).  tab = [Gt | Ht] in shared memory.
+//   fast path (ng % 8 == 0, ng - P >= 8): the support meets the brick in one run, brick-local j <-> r = r0 + j
+//   generic path: direct exp per point, periodic wrap per point
 template <bool FIELD>
-__device__ __forceinline__ void brick_weights(const WaveConst& wc, const double* __restrict__ Gs, int b0, int ng, int s0, double e0,
-                                              double e1, double u0, double scale, double* __restrict__ w)
+__device__ __forceinline__ void brick_weights(const WaveConst& wc, const double* __restrict__ tab, bool generic, int b0, int ng,
+                                              int s0, const double4 cf, double u0, double scale, double* __restrict__ w)
 {
     const int P = wc.P;
     const int dsl = wrap_once(b0 - s0, ng);
-    double pw = 0.0;
-    if (dsl < P) {  // e0 e1^dsl
-        double r = e0, b = e1;
-        int n = dsl;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            if (n & 1) r *= b;
-            b *= b;
-            n >>= 1;
-        }
-        pw = r;
-    }
-    int r = dsl;
     double v[BR], vu[BR];
+    if (!generic) {
+        const int r0 = (dsl < P) ? dsl : dsl - ng;
+        const int phi = (-s0) & (BR - 1);
+        const int m = (r0 - phi) >> 3;  // -1 .. 3
+        const double e82 = cf.z * cf.z;
+        const double pm = (m < 0) ? cf.w : (m == 0) ? 1.0 : (m == 1) ? cf.z : (m == 2) ? e82 : e82 * cf.z;
+        double pw = cf.x * pm * tab[r0 + 8] * scale;
+        double t = cf.y * tab[48 + r0 + 8];
+        const double g2 = tab[9] * tab[9];  // exp(-2 aw)
 #pragma unroll
-    for (int j = 0; j < BR; ++j) {
-        const bool in = r < P;
-        const double g = Gs[in ? r : 0];
-        v[j] = in ? pw * g * scale : 0.0;
-        if (FIELD) vu[j] = v[j] * (u0 + (double)r);
-        pw *= e1;
-        ++r;
-        if (r == ng) { r = 0; pw = e0; }
+        for (int j = 0; j < BR; ++j) {
+            const int r = r0 + j;
+            v[j] = (r >= 0 && r < P) ? pw : 0.0;
+            if (FIELD) vu[j] = v[j] * (u0 + (double)r);
+            pw *= t;
+            t *= g2;
+        }
+    } else {
+        int r = dsl;
+#pragma unroll
+        for (int j = 0; j < BR; ++j) {
+            const double u = u0 + (double)r;
+            v[j] = (r < P) ? scale * exp(-wc.aw * u * u) : 0.0;
+            if (FIELD) vu[j] = v[j] * u;
+            if (++r == ng) r = 0;
+        }
     }
 #pragma unroll
     for (int j = 0; j < BR; j += 2) *reinterpret_cast<double2*>(w + j) = make_double2(v[j], v[j + 1]);
@@ -177,16 +178,27 @@ __device__ __forceinline__ void brick_weights(const WaveConst& wc, const double*
     }
 }
 
-// hits appended by the test phase; process() consumes the first min(nq, 32)
+__device__ __forceinline__ void load_tables(const WaveConst& wc, double* tab)
+{
+    for (int k = threadIdx.x; k < NTAB; k += blockDim.x) {
+        const int r = (k < 48 ? k : k - 48) - 8;
+        tab[k] = (k < 48) ? exp(-wc.aw * (double)(r * r)) : exp(-wc.aw * (double)(2 * r + 1));
+    }
+    __syncthreads();
+}
+
+// hits appended by the test phase; PROCESS consumes the first min(nq, 32).  Each lane walks the runs forwards:
+// its candidates c = lane, lane + 32, ... only ever move to later runs.
 #define BRICK_WALK(PROCESS)                                                                        \
-    int nq = 0;                                                                                    \
+    int nq = 0, pc = 0;                                                                            \
     for (int cb = 0; cb < br.M; cb += 32) {                                                        \
         const int c = cb + lane;                                                                   \
         bool hit = false;                                                                          \
         int pi = 0;                                                                                \
         if (c < br.M) {                                                                            \
-            pi = candidate_slot(s, br.npiece, c);                                                  \
-            hit = support_meets_brick(wc, br, wp, pi);                                             \
+            while (c >= s.p_prefix[pc + 1]) ++pc;                                                  \
+            pi = s.p_start[pc] + (c - s.p_prefix[pc]);                                             \
+            hit = support_meets_brick(wc, br, wp.s0[pi]);                                          \
         }                                                                                          \
         const unsigned m = __ballot_sync(0xffffffffu, hit);                                        \
         if (hit) s.qidx[nq + __popc(m & ((1u << lane) - 1u))] = pi;                                \
@@ -207,37 +219,57 @@ __device__ __forceinline__ void brick_weights(const WaveConst& wc, const double*
 // ---------------------------------------------------------------- window coefficients (once per position update)
 __global__ void __launch_bounds__(256)
 k_window_coef(int n, WaveConst wc, const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
-              int* __restrict__ s0x, int* __restrict__ s0y, int* __restrict__ s0z, double* __restrict__ e0x, double* __restrict__ e0y,
-              double* __restrict__ e0z, double* __restrict__ e1x, double* __restrict__ e1y, double* __restrict__ e1z)
+              int4* __restrict__ s0o, double4* __restrict__ cfo)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double pos[3] = {xs[i], ys[i], zs[i]};
-    int* so[3] = {s0x, s0y, s0z};
-    double* a0[3] = {e0x, e0y, e0z};
-    double* a1[3] = {e1x, e1y, e1z};
+    int sv[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const double xd = pos[d] * wc.inv_h[d];
         const int i0 = min((int)xd, wc.Ng[d] - 1);
         const int s0 = i0 - wc.P / 2 + 1;  // first support index (reading A5, even P); may be negative
         const double u0 = (double)s0 - xd; // in (-P/2, -P/2 + 1]
-        so[d][i] = s0;
-        a0[d][i] = exp(-wc.aw * u0 * u0);
-        a1[d][i] = exp(-2.0 * wc.aw * u0);
+        const int phi = (-s0) & (BR - 1);
+        sv[d] = s0;
+        cfo[3 * (size_t)i + d] = make_double4(exp(-wc.aw * u0 * (u0 + 2.0 * phi)), exp(-2.0 * wc.aw * u0), exp(-16.0 * wc.aw * u0),
+                                              exp(16.0 * wc.aw * u0));
     }
+    s0o[i] = make_int4(sv[0], sv[1], sv[2], 0);
 }
 
+// weights of the first nh queued hits, one hit per lane, into the warp's table
+#define BRICK_WEIGHTS(FIELD_, STRIDE_, DW_, QSCALE)                                                                     \
+    if (lane < nh) {                                                                                                    \
+        const int p = s.qidx[lane];                                                                                     \
+        double* w = s.wt + lane * (STRIDE_);                                                                            \
+        const int4 s0v = wp.s0[p];                                                                                      \
+        const int sv[3] = {s0v.x, s0v.y, s0v.z};                                                                        \
+        double u0[3] = {0.0, 0.0, 0.0};                                                                                 \
+        if ((FIELD_) || generic) {                                                                                      \
+            u0[0] = (double)sv[0] - xs[p] * wc.inv_h[0];                                                                \
+            u0[1] = (double)sv[1] - ys[p] * wc.inv_h[1];                                                                \
+            u0[2] = (double)sv[2] - zs[p] * wc.inv_h[2];                                                                \
+        }                                                                                                               \
+        const double qscale = (QSCALE);                                                                                 \
+        _Pragma("unroll") for (int d = 0; d < 3; ++d)                                                                   \
+            brick_weights<FIELD_>(wc, tab, generic, br.b0[d], wc.Ng[d], sv[d], wp.cf[3 * (size_t)p + d], u0[d],         \
+                                  d == 2 ? qscale : 1.0, w + (DW_) * d);                                                \
+    }                                                                                                                   \
+    __syncwarp();
+
 // ---------------------------------------------------------------- spread
-__global__ void __launch_bounds__(BWARPS * 32)
+__global__ void __launch_bounds__(BWARPS * 32, 5)
 k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
-                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok)
+                const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* Gs = reinterpret_cast<double*>(smem_raw);
-    WarpSmem<STRIDE_PSI>* sm = reinterpret_cast<WarpSmem<STRIDE_PSI>*>(smem_raw + 32 * sizeof(double));
-    if (threadIdx.x < 32) Gs[threadIdx.x] = wc.G[threadIdx.x];
-    __syncthreads();
+    double* tab = reinterpret_cast<double*>(smem_raw);
+    WarpSmem<STRIDE_PSI>* sm = reinterpret_cast<WarpSmem<STRIDE_PSI>*>(smem_raw + NTAB * sizeof(double));
+    load_tables(wc, tab);
+    const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE_PSI>& s = sm[warp];
     Brick br;
@@ -252,15 +284,7 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 #define SPREAD_PROCESS(NH)                                                                                              \
     {                                                                                                                   \
         const int nh = (NH);                                                                                            \
-        if (lane < nh) {                                                                                                \
-            const int p = s.qidx[lane];                                                                                 \
-            const double qv = qs[p];                                                                                    \
-            double* w = s.wt + lane * STRIDE_PSI;                                                                       \
-            _Pragma("unroll") for (int d = 0; d < 3; ++d)                                                               \
-                brick_weights<false>(wc, Gs, br.b0[d], wc.Ng[d], wp.s0[d][p], wp.e0[d][p], wp.e1[d][p], 0.0,            \
-                                     d == 2 ? qv : 1.0, w + BR * d);                                                    \
-        }                                                                                                               \
-        __syncwarp();                                                                                                   \
+        BRICK_WEIGHTS(false, STRIDE_PSI, BR, qs[p])                                                                     \
         for (int slot = 0; slot < nh; ++slot) {                                                                         \
             const double* w = s.wt + slot * STRIDE_PSI;                                                                 \
             const double2 x01 = *reinterpret_cast<const double2*>(w + px);                                              \
@@ -298,7 +322,6 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
         }
     }
 }
-
 // ---------------------------------------------------------------- gather
 // reduce NV values per lane across the warp; afterwards lanes with (lane & (32/NV - 1)) == 0 hold the warp
 // total of value number `id`
@@ -325,21 +348,21 @@ __device__ __forceinline__ double transpose_reduce(double (&v)[NV], int lane, in
 }
 
 template <bool FIELD>
-__global__ void __launch_bounds__(BWARPS * 32)
+__global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 5)
 k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                 const double* __restrict__ grid, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
-                double* __restrict__ ez, int vec_ok)
+                double* __restrict__ ez, int vec_ok, int generic_)
 {
     constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
     constexpr int DW = FIELD ? 2 * BR : BR;  // doubles per dimension in the weight table
     constexpr int G = FIELD ? 4 : 8;         // hits per butterfly
     constexpr int NQ = FIELD ? 4 : 1;        // quantities per hit: psi (, Ex, Ey, Ez)
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* Gs = reinterpret_cast<double*>(smem_raw);
-    WarpSmem<STRIDE>* sm = reinterpret_cast<WarpSmem<STRIDE>*>(smem_raw + 32 * sizeof(double));
-    if (threadIdx.x < 32) Gs[threadIdx.x] = wc.G[threadIdx.x];
-    __syncthreads();
+    double* tab = reinterpret_cast<double*>(smem_raw);
+    WarpSmem<STRIDE>* sm = reinterpret_cast<WarpSmem<STRIDE>*>(smem_raw + NTAB * sizeof(double));
+    load_tables(wc, tab);
+    const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE>& s = sm[warp];
     Brick br;
@@ -369,17 +392,7 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 #define GATHER_PROCESS(NH)                                                                                              \
     {                                                                                                                   \
         const int nh = (NH);                                                                                            \
-        if (lane < nh) {                                                                                                \
-            const int p = s.qidx[lane];                                                                                 \
-            double* w = s.wt + lane * STRIDE;                                                                           \
-            const double pos[3] = {FIELD ? xs[p] : 0.0, FIELD ? ys[p] : 0.0, FIELD ? zs[p] : 0.0};                      \
-            _Pragma("unroll") for (int d = 0; d < 3; ++d) {                                                             \
-                const int s0 = wp.s0[d][p];                                                                             \
-                const double u0 = FIELD ? (double)s0 - pos[d] * wc.inv_h[d] : 0.0;                                      \
-                brick_weights<FIELD>(wc, Gs, br.b0[d], wc.Ng[d], s0, wp.e0[d][p], wp.e1[d][p], u0, 1.0, w + DW * d);    \
-            }                                                                                                           \
-        }                                                                                                               \
-        __syncwarp();                                                                                                   \
+        BRICK_WEIGHTS(FIELD, STRIDE, DW, 1.0)                                                                           \
         for (int sb = 0; sb < nh; sb += G) {                                                                            \
             double v[NQ * G];                                                                                           \
             _Pragma("unroll") for (int g = 0; g < G; ++g) {                                                             \
@@ -441,7 +454,7 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 // ---------------------------------------------------------------- host
 static size_t smem_bytes(bool field)
 {
-    return 32 * sizeof(double) + BWARPS * (field ? sizeof(WarpSmem<STRIDE_FLD>) : sizeof(WarpSmem<STRIDE_PSI>));
+    return NTAB * sizeof(double) + BWARPS * (field ? sizeof(WarpSmem<STRIDE_FLD>) : sizeof(WarpSmem<STRIDE_PSI>));
 }
 
 int wave_bricks_init(pce_ctx* c)
@@ -455,12 +468,9 @@ int wave_bricks_init(pce_ctx* c)
 int wave_coef_alloc(pce_ctx* c, Bins& b)
 {
     const size_t n = (size_t)(b.n > 0 ? b.n : 1);
-    for (int d = 0; d < 3; ++d) {
-        PCE_CUDA(c, cudaMalloc(&b.ws0[d], n * sizeof(int)));
-        PCE_CUDA(c, cudaMalloc(&b.we0[d], n * sizeof(double)));
-        PCE_CUDA(c, cudaMalloc(&b.we1[d], n * sizeof(double)));
-    }
-    c->bytes += (long long)(n * 60);
+    PCE_CUDA(c, cudaMalloc(&b.ws0, n * sizeof(int4)));
+    PCE_CUDA(c, cudaMalloc(&b.wcf, 3 * n * sizeof(double4)));
+    c->bytes += (long long)(n * 112);
     return PCE_OK;
 }
 
@@ -468,8 +478,7 @@ int wave_coef_alloc(pce_ctx* c, Bins& b)
 int wave_window_coef(pce_ctx* c, const Bins& b)
 {
     if (b.n == 0) return PCE_OK;
-    k_window_coef<<<cdiv(b.n, 256), 256, 0, c->st>>>(b.n, c->wk, b.xs, b.ys, b.zs, b.ws0[0], b.ws0[1], b.ws0[2], b.we0[0], b.we0[1],
-                                                     b.we0[2], b.we1[0], b.we1[1], b.we1[2]);
+    k_window_coef<<<cdiv(b.n, 256), 256, 0, c->st>>>(b.n, c->wk, b.xs, b.ys, b.zs, b.ws0, b.wcf);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -478,8 +487,16 @@ int wave_window_coef(pce_ctx* c, const Bins& b)
 static WinCoefPtrs coef_ptrs(const Bins& b)
 {
     WinCoefPtrs p;
-    for (int d = 0; d < 3; ++d) { p.s0[d] = b.ws0[d]; p.e0[d] = b.we0[d]; p.e1[d] = b.we1[d]; }
+    p.s0 = b.ws0; p.cf = b.wcf;
     return p;
+}
+
+// the fast weight routine needs bricks aligned with the periodic mesh and a support that meets a brick in one run
+static int generic_weights(const pce_ctx* c)
+{
+    for (int d = 0; d < 3; ++d)
+        if (c->wk.Ng[d] % BR != 0 || c->wk.Ng[d] - c->wk.P < BR) return 1;
+    return 0;
 }
 
 int wave_spread_bricks(pce_ctx* c, const Bins& b)
@@ -487,7 +504,7 @@ int wave_spread_bricks(pce_ctx* c, const Bins& b)
     PassTimer t(c, PASS_SPREAD);
     const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
     k_spread_bricks<<<cdiv(b.ncell, BWARPS), BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
-                                                                                     coef_ptrs(b), b.qs, c->grid, vec_ok);
+                                                                                     coef_ptrs(b), b.xs, b.ys, b.zs, b.qs, c->grid, vec_ok, generic_weights(c));
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -506,11 +523,11 @@ int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, dou
         PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
         k_gather_bricks<true><<<blocks, BWARPS * 32, smem_bytes(true), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, ex_s, ey_s,
-                                                                               ez_s, vec_ok);
+                                                                               ez_s, vec_ok, generic_weights(c));
     } else {
         k_gather_bricks<false><<<blocks, BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                  coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, nullptr,
-                                                                                 nullptr, nullptr, vec_ok);
+                                                                                 nullptr, nullptr, vec_ok, generic_weights(c));
     }
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
