@@ -91,7 +91,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     cudaStreamSynchronize(c->st);
     free_system(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;

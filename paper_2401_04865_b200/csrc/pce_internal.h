@@ -102,6 +102,9 @@ struct pce_ctx {
     cufftHandle planF = 0, planB = 0;
     void* fft_work = nullptr;
     bool have_plans = false;
+    // persistent brick kernels (wave_bricks.cu)
+    int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
+    int* work_ctr = nullptr;
 
     // per-call work vectors
     double *w_real = nullptr, *w_wave = nullptr;            // [N] sorted-order potentials

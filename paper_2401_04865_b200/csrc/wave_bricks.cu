@@ -263,7 +263,7 @@ k_window_coef(int n, WaveConst wc, const double* __restrict__ xs, const double* 
 __global__ void __launch_bounds__(BWARPS * 32, 5)
 k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
-                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_)
+                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_, int* __restrict__ work_ctr)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* tab = reinterpret_cast<double*>(smem_raw);
@@ -272,9 +272,13 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE_PSI>& s = sm[warp];
-    Brick br;
-    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, blockIdx.x * BWARPS + warp)) return;
     const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    for (;;) {  // persistent warps: bricks are handed out by a global counter
+    int brick_id = 0;
+    if (lane == 0) brick_id = atomicAdd(work_ctr, 1);
+    brick_id = __shfl_sync(0xffffffffu, brick_id, 0);
+    Brick br;
+    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, brick_id)) return;
     double acc[4][4];
 #pragma unroll
     for (int j = 0; j < 4; ++j)
@@ -304,13 +308,12 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 #undef SPREAD_PROCESS
 
     const int gz = br.b0[2] + pz;
-    if (gz >= wc.Ng[2]) return;
     const size_t Nx = wc.Ng[0], Ny = wc.Ng[1];
     const int gx = br.b0[0] + px;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int gy = br.b0[1] + py + j;
-        if (gy >= wc.Ng[1]) break;
+        if (gz >= wc.Ng[2] || gy >= wc.Ng[1]) break;
         double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
         if (vec_ok && gx + 3 < wc.Ng[0]) {
             *reinterpret_cast<double2*>(row) = make_double2(acc[j][0], acc[j][1]);
@@ -321,6 +324,8 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
                 if (gx + i < wc.Ng[0]) row[i] = acc[j][i];
         }
     }
+    __syncwarp();
+    }  // next brick
 }
 // ---------------------------------------------------------------- gather
 // reduce NV values per lane across the warp; afterwards lanes with (lane & (32/NV - 1)) == 0 hold the warp
@@ -352,7 +357,7 @@ __global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 5)
 k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                 const double* __restrict__ grid, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
-                double* __restrict__ ez, int vec_ok, int generic_)
+                double* __restrict__ ez, int vec_ok, int generic_, int* __restrict__ work_ctr)
 {
     constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
     constexpr int DW = FIELD ? 2 * BR : BR;  // doubles per dimension in the weight table
@@ -365,10 +370,14 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE>& s = sm[warp];
-    Brick br;
-    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, blockIdx.x * BWARPS + warp)) return;
-    if (br.M == 0) return;
     const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    for (;;) {  // persistent warps: bricks are handed out by a global counter
+    int brick_id = 0;
+    if (lane == 0) brick_id = atomicAdd(work_ctr, 1);
+    brick_id = __shfl_sync(0xffffffffu, brick_id, 0);
+    Brick br;
+    if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, brick_id)) return;
+    if (br.M == 0) continue;
     // the lane's 4x4 patch of H~ in registers (0 outside the mesh)
     double H[4][4];
     {
@@ -449,6 +458,8 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 
     BRICK_WALK(GATHER_PROCESS)
 #undef GATHER_PROCESS
+    __syncwarp();
+    }  // next brick
 }
 
 // ---------------------------------------------------------------- host
@@ -462,6 +473,14 @@ int wave_bricks_init(pce_ctx* c)
     PCE_CUDA(c, cudaFuncSetAttribute(k_spread_bricks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(false)));
     PCE_CUDA(c, cudaFuncSetAttribute(k_gather_bricks<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(false)));
     PCE_CUDA(c, cudaFuncSetAttribute(k_gather_bricks<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(true)));
+    int dev = 0;
+    PCE_CUDA(c, cudaGetDevice(&dev));
+    PCE_CUDA(c, cudaDeviceGetAttribute(&c->num_sm, cudaDevAttrMultiProcessorCount, dev));
+    PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_spread, k_spread_bricks, BWARPS * 32, smem_bytes(false)));
+    PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gather, k_gather_bricks<false>, BWARPS * 32, smem_bytes(false)));
+    PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_gather_f, k_gather_bricks<true>, BWARPS * 32, smem_bytes(true)));
+    if (c->occ_spread < 1 || c->occ_gather < 1 || c->occ_gather_f < 1) { c->err = "brick kernels do not fit on this device"; return PCE_ECUDA; }
+    PCE_CUDA(c, cudaMalloc(&c->work_ctr, 4 * sizeof(int)));
     return PCE_OK;
 }
 
@@ -499,12 +518,20 @@ static int generic_weights(const pce_ctx* c)
     return 0;
 }
 
+// persistent grid: as many CTAs as fit on the device (occupancy query at init), never more than there are bricks
+static int grid_for(const pce_ctx* c, int per_sm, int nbrick)
+{
+    const int want = c->num_sm * per_sm, need = cdiv(nbrick, BWARPS);
+    return want < need ? want : need;
+}
+
 int wave_spread_bricks(pce_ctx* c, const Bins& b)
 {
     PassTimer t(c, PASS_SPREAD);
     const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
-    k_spread_bricks<<<cdiv(b.ncell, BWARPS), BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
-                                                                                     coef_ptrs(b), b.xs, b.ys, b.zs, b.qs, c->grid, vec_ok, generic_weights(c));
+    PCE_CUDA(c, cudaMemsetAsync(c->work_ctr, 0, sizeof(int), c->st));
+    k_spread_bricks<<<grid_for(c, c->occ_spread, b.ncell), BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
+                                                                                     coef_ptrs(b), b.xs, b.ys, b.zs, b.qs, c->grid, vec_ok, generic_weights(c), c->work_ctr);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -515,7 +542,8 @@ int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, dou
     if (b.n == 0) return PCE_OK;
     PassTimer t(c, PASS_GATHER);
     const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
-    const int blocks = cdiv(b.ncell, BWARPS);
+    const int blocks = grid_for(c, field ? c->occ_gather_f : c->occ_gather, b.ncell);
+    PCE_CUDA(c, cudaMemsetAsync(c->work_ctr, 0, sizeof(int), c->st));
     PCE_CUDA(c, cudaMemsetAsync(psi_s, 0, (size_t)b.n * sizeof(double), c->st));
     if (field) {
         PCE_CUDA(c, cudaMemsetAsync(ex_s, 0, (size_t)b.n * sizeof(double), c->st));
@@ -523,11 +551,11 @@ int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, dou
         PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
         k_gather_bricks<true><<<blocks, BWARPS * 32, smem_bytes(true), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, ex_s, ey_s,
-                                                                               ez_s, vec_ok, generic_weights(c));
+                                                                               ez_s, vec_ok, generic_weights(c), c->work_ctr);
     } else {
         k_gather_bricks<false><<<blocks, BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                  coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, nullptr,
-                                                                                 nullptr, nullptr, vec_ok, generic_weights(c));
+                                                                                 nullptr, nullptr, vec_ok, generic_weights(c), c->work_ctr);
     }
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
