@@ -1,0 +1,123 @@
+"""GPU parity at BASELINE.json's full sizes (configs 4 and 5), in the launch configuration bench.py times.
+
+A full-vector oracle solve is infeasible there, so the CUDA path is checked
+  (i)   on SAMPLED outputs the oracle can compute one by one: potential and field of the GPU's final charges
+        at S random beads and ions from ALL sources (direct Ewald sum, eq. 19);
+  (ii)  via properties that hold at any size and single out the unique solution of eq. 13 (M is SPD,
+        PAPER.md:99): sum_j q_ij = Q_i, and psi_ij - r_ij.E0 = Phi_i on every sampled bead, with psi from the ORACLE;
+  (iii) on a density-matched replica of config 5 (8 spheroids + 16 000 ions, same h) with full-vector parity.
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-9
+TOL_FORCE = 1e-8
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def pce():
+    import torch
+    import paper_2401_04865_b200 as p
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    p.build()
+    return p
+
+
+def _sampled_parity(pce, w, n_bead_s, n_ion_s, seed):
+    ctx = pce.context_for(w)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    qn, Phin = q.cpu().numpy(), Phi.cpu().numpy()
+    psi_g, f_g = out["psi"].cpu().numpy(), out["f"].cpu().numpy()
+    _, ex, ey, ez = ctx.evaluate(q)
+    E_all = np.stack([ex.cpu().numpy(), ey.cpu().numpy(), ez.cpu().numpy()], axis=1)
+    ctx.close()
+    assert info["converged"], info
+    off = np.asarray(w.body_offset)
+    # constraints (eq. 11): exact up to rounding of a ~1000-term sum
+    Qg = np.add.reduceat(qn[:w.N_bead], off[:-1])
+    assert np.abs(Qg - w.Q_body).max() < 1e-11 * max(1.0, np.abs(qn[:w.N_bead]).max() * 1000)
+    assert np.array_equal(qn[w.N_bead:], w.q_ion)
+    rng = np.random.default_rng(seed)
+    tb = np.sort(rng.choice(w.N_bead, size=n_bead_s, replace=False))
+    ti = np.sort(w.N_bead + rng.choice(w.N_ion, size=n_ion_s, replace=False))
+    tg = np.concatenate([tb, ti])
+    psi_o, E_o = orc.ewald_eval(w.x, qn, w.L, w.a, w.eps_f, targets=tg, field=True)
+    f_o = qn[tg, None] * (np.asarray(w.E0)[None, :] + E_o)
+    res = {"psi": rel(psi_g[tg], psi_o), "f": rel(f_g[tg], f_o), "iters": info["iters"]}
+    res["E"] = rel(E_all[tg], E_o)
+    # KKT rows at the sampled beads: psi_oracle - r.E0 - Phi_body = 0 (eq. 12)
+    _, r = orc.body_centres(w.x, off, w.L)
+    body = np.searchsorted(off, tb, side="right") - 1
+    kkt = psi_o[:n_bead_s] - r[tb] @ np.asarray(w.E0) - Phin[body]
+    scale = np.sqrt(np.mean((r[tb] @ np.asarray(w.E0)) ** 2) + np.mean(psi_o[:n_bead_s] ** 2))
+    res["kkt"] = float(np.sqrt(np.mean(kkt ** 2)) / scale)
+    return res
+
+
+def test_config4_lattice_sampled_targets(pce):
+    """config 4: 64 spheres x 642 beads + 100 000 ions, 256^3."""
+    w = wl.config4()
+    r = _sampled_parity(pce, w, 96, 96, seed=41)
+    assert r["psi"] < TOL_FIELD and r["E"] < TOL_FIELD and r["f"] < TOL_FORCE and r["kkt"] < TOL_FIELD, r
+
+
+def test_config4_no_ions_lattice_symmetry(pce):
+    """Pin P12 on the CUDA path: identical spheres on a simple-cubic lattice carry identical dipoles, no force or
+    torque, equal potentials (C_qE = C_S.Psi = 0 by symmetry)."""
+    w = wl.config4(with_ions=False)
+    ctx = pce.context_for(w)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    S, F, T = out["S"].cpu().numpy(), out["F"].cpu().numpy(), out["T"].cpu().numpy()
+    fmax = np.abs(out["f"].cpu().numpy()).sum(0).max()
+    ctx.close()
+    assert info["converged"]
+    assert np.abs(S - S.mean(0)).max() < 1e-8 * np.abs(S).max()
+    assert np.abs(F).max() < 1e-8 * fmax and np.abs(T).max() < 1e-8 * fmax
+    ph = Phi.cpu().numpy()
+    assert np.abs(ph - ph.mean()).max() < 1e-9 * max(np.abs(q.cpu().numpy()).max(), 1.0)
+
+
+def test_config5_replica_full_parity(pce):
+    """Density-matched replica of config 5 (8 spheroids x 1000 beads + 16 000 ions, 128^3, same mesh spacing):
+    full-vector parity of charges, potentials, forces, torques (oracle: CG with the direct Ewald matvec)."""
+    w = wl.config5_replica()
+    ctx = pce.context_for(w)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    ctx.close()
+    qo, Phio, oinfo = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a, w.eps_f, method="cg")
+    oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, w.eps_f, Phi_body=Phio)
+    fscale = np.abs(oo["f"]).sum(0).max()
+    r = {"q": rel(q.cpu().numpy(), qo), "psi": rel(out["psi"].cpu().numpy(), oo["psi"]), "f": rel(out["f"].cpu().numpy(), oo["f"]),
+         "Phi": float(np.abs(Phi.cpu().numpy() - Phio).max() / np.abs(oo["psi"]).max()),
+         "F": float(np.abs(out["F"].cpu().numpy() - oo["F"]).max() / fscale),
+         "T": float(np.abs(out["T"].cpu().numpy() - oo["T"]).max() / fscale),
+         "S": rel(out["S"].cpu().numpy(), oo["S"])}
+    assert info["converged"]
+    assert r["q"] < TOL_FIELD and r["psi"] < TOL_FIELD and r["Phi"] < TOL_FIELD and r["S"] < TOL_FIELD, r
+    assert r["f"] < TOL_FORCE and r["F"] < TOL_FORCE and r["T"] < TOL_FORCE, r
+
+
+def test_config5_full_size_sampled_targets(pce):
+    """config 5 at full size (500 000 beads + 1 000 000 ions, 512^3), as bench.py runs it."""
+    w = wl.config5()
+    r = _sampled_parity(pce, w, 48, 48, seed=51)
+    assert r["psi"] < TOL_FIELD and r["E"] < TOL_FIELD and r["f"] < TOL_FORCE and r["kkt"] < TOL_FIELD, r
