@@ -54,6 +54,9 @@ typedef enum {
     PCE_ESTATE = -6    /* call order violated (e.g. solve before set_system) */
 } pce_status;
 
+/* pce_params.flags */
+#define PCE_FLAG_NO_PRECOND 1  /* plain (unpreconditioned) conjugate gradients in pce_solve */
+
 /* Parameters of the spectral Ewald sum and of the solver.
  * eta is NOT a free input: eta = h^2 xi^2 P / pi (eq. 31,
  * PAPER.md:250), per dimension for a rectangular box. */
@@ -67,7 +70,7 @@ typedef struct {
     double eps_f;       /* fluid permittivity (1 in the paper's units) */
     double tol_solver;  /* relative residual at which the Krylov solve stops */
     int    max_iter;    /* iteration cap of the Krylov solve */
-    int    flags;       /* reserved, 0 */
+    int    flags;       /* 0, or PCE_FLAG_* ORed */
 } pce_params;
 
 typedef struct {
@@ -96,6 +99,8 @@ typedef struct {
     long long nnz_near;     /* entries of the cached bead-bead near field */
     int    N, N_bead, N_body;
     long long bytes_workspace;
+    long long bytes_precond; /* fp32 storage of the block-Jacobi preconditioner (0: off) */
+    int n_precond_blocks;    /* bodies that own a dense preconditioner block */
 } pce_info;
 
 /* Ewald parameters from a target tolerance (pure host arithmetic):
@@ -144,7 +149,13 @@ int pce_evaluate(pce_ctx* ctx, const double* q, double* psi,
  *           warm_start != 0 its bead part is read as the initial guess.
  *  Phi_body : device [N_body] out.
  * Method: conjugate gradients on the per-body-mean-projected SPD system,
- * whole iteration on the device.  Returns PCE_ENOCONV if max_iter was hit. */
+ * whole iteration on the device, preconditioned (unless PCE_FLAG_NO_PRECOND)
+ * by the inverse of each body's own free-space potential tensor (eq. 10) on
+ * its zero-net-charge subspace.  That block depends on the body-frame bead
+ * positions only, so it is built once in pce_set_system and stays valid while
+ * pce_set_positions moves the bodies rigidly; a non-rigid
+ * update costs iterations, never accuracy (the solution of eq. 13 is unique).
+ * Returns PCE_ENOCONV if max_iter was hit. */
 int pce_solve(pce_ctx* ctx, const double* Q_body, const double* q_ion, const double E0[3],
               int warm_start, double* q, double* Phi_body, pce_solve_info* info);
 

@@ -47,7 +47,7 @@ class PceTimings(C.Structure):
 class PceInfo(C.Structure):
     _fields_ = [("eta", C.c_double * 3), ("h", C.c_double * 3), ("ncell", C.c_int * 3), ("image_range", C.c_int * 3),
                 ("nnz_near", C.c_longlong), ("N", C.c_int), ("N_bead", C.c_int), ("N_body", C.c_int),
-                ("bytes_workspace", C.c_longlong)]
+                ("bytes_workspace", C.c_longlong), ("bytes_precond", C.c_longlong), ("n_precond_blocks", C.c_int)]
 
 
 class PceError(RuntimeError):
@@ -238,15 +238,20 @@ class Context:
         i = PceInfo()
         self._ck(self.lib.pce_get_info(self.h, C.byref(i)))
         return {"eta": list(i.eta), "h": list(i.h), "ncell": list(i.ncell), "image_range": list(i.image_range),
-                "nnz_near": i.nnz_near, "N": i.N, "N_bead": i.N_bead, "N_body": i.N_body, "bytes_workspace": i.bytes_workspace}
+                "nnz_near": i.nnz_near, "N": i.N, "N_bead": i.N_bead, "N_body": i.N_body, "bytes_workspace": i.bytes_workspace,
+                "bytes_precond": i.bytes_precond, "n_precond_blocks": i.n_precond_blocks}
 
     def launch_count(self):
         return int(self.lib.pce_launch_count(self.h))
 
 
-def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None) -> Context:
+PCE_FLAG_NO_PRECOND = 1
+
+
+def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None, precond=True) -> Context:
     """Context with parameters suggested for a workloads.Workload."""
     p = suggest_params(workload.L, workload.Ng, workload.a, tol, P)
+    p.flags = 0 if precond else PCE_FLAG_NO_PRECOND
     p.eps_f = workload.eps_f
     p.tol_solver = tol_solver
     p.max_iter = max_iter

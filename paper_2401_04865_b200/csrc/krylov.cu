@@ -149,7 +149,7 @@ k_proj_dot(const int* __restrict__ off, const double* __restrict__ t, const doub
     if (threadIdx.x == 0) part[b] = d;
 }
 
-// alpha = gg/pAp ; q += alpha p ; g -= alpha ap ; psi += alpha t ; partial of |g|^2
+// alpha = (g.z)/pAp ; q += alpha p ; g -= alpha ap ; psi += alpha t ; partial of |g|^2
 __global__ void __launch_bounds__(BT)
 k_cg_update(const int* __restrict__ off, const double* __restrict__ sc_gg, const double* __restrict__ sc_pap,
             const double* __restrict__ p, const double* __restrict__ ap, const double* __restrict__ t, double* __restrict__ q,
@@ -172,15 +172,36 @@ k_cg_update(const int* __restrict__ off, const double* __restrict__ sc_gg, const
     if (threadIdx.x == 0) part[b] = gg;
 }
 
-// beta = gg_new/gg_old ; p = g + beta p
-__global__ void k_cg_pupdate(int n, const double* __restrict__ sc_gg_old, const double* __restrict__ sc_gg_new,
-                             const double* __restrict__ g, double* __restrict__ p)
+// beta = rz_new/rz_old (0 on the first call) ; p = z + beta p with z = g (no preconditioner) or
+// z = z_raw - <z_raw>_body (block-Jacobi, precond.cu)
+__global__ void k_cg_pupdate(int n, const double* __restrict__ sc_old, const double* __restrict__ sc_new, const double* __restrict__ g,
+                             const double* __restrict__ zraw, const double* __restrict__ zmean, const int* __restrict__ body_of,
+                             double* __restrict__ p)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const double o = sc_gg_old[0];
-    const double beta = (o != 0.0) ? sc_gg_new[0] / o : 0.0;
-    p[i] = g[i] + beta * p[i];
+    double beta = 0.0;
+    if (sc_old) {
+        const double o = sc_old[0];
+        beta = (o != 0.0) ? sc_new[0] / o : 0.0;
+    }
+    const double z = zraw ? zraw[i] - zmean[body_of[i]] : g[i];
+    p[i] = sc_old ? z + beta * p[i] : z;
+}
+
+// per body: mean of z_raw and the partial of g.z (g has zero mean per body, so g.z = g.z_raw)
+__global__ void __launch_bounds__(BT)
+k_pc_dot(const int* __restrict__ off, const double* __restrict__ zraw, const double* __restrict__ g, double* __restrict__ zmean,
+         double* __restrict__ part)
+{
+    __shared__ double sh[32];
+    const int b = blockIdx.x;
+    const int j0 = off[b], j1 = off[b + 1];
+    double s = 0.0, d = 0.0;
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) { const double z = zraw[j]; s += z; d += g[j] * z; }
+    s = block_sum(s, sh);
+    d = block_sum(d, sh);
+    if (threadIdx.x == 0) { zmean[b] = (j1 > j0) ? s / (j1 - j0) : 0.0; part[b] = d; }
 }
 
 // Phi_i = <psi_ij - r_ij.E0>_i = <psi_ij>_i
@@ -222,30 +243,42 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
     if (rc) return rc;
     inf.matvecs = 1;
     const int maxit = c->p.max_iter;
-    double* sc = c->cg_scal;          // [0]=ref^2, then per iteration it: gg at 2+2it, pAp at 3+2it
-    double* part = c->cg_scal + 2 * (maxit + 2) + 2;  // [nb] partials
+    // device scalars: [0] = ref^2, [1] = |g_0|^2; iteration it: g.z at 2+3it, p.Ap at 3+3it, |g_{it+1}|^2 at 4+3it
+    double* sc = c->cg_scal;
+    double* part = c->cg_scal + 3 * (maxit + 2) + 2;  // [nb] partials
     double* part2 = part + nb;
+    const bool pc = c->pc_on;
+    const double* zraw = pc ? c->cg_z : nullptr;
+    double* cur_rz = pc ? sc + 2 : sc + 1;
     {
         PassTimer t(c, PASS_KRYLOV);
         k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->ev_psi, c->cg_psi);
         k_resid_init<<<nb, BT, 0, c->st>>>(c->body_off, c->rx, c->ry, c->rz, E0[0], E0[1], E0[2], c->ev_psi, c->cg_rhs, c->cg_g,
                                          c->cg_p, part, part2);
         c->launches += 2;
-        if ((rc = sum_to(c, part, nb, sc + 2))) return rc;
+        if ((rc = sum_to(c, part, nb, sc + 1))) return rc;
         if ((rc = sum_to(c, part2, nb, sc + 0))) return rc;
+        if (pc) {
+            if ((rc = precond_apply(c, c->cg_g, c->cg_z))) return rc;
+            k_pc_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_z, c->cg_g, c->pc_mean, part);
+            c->launches++;
+            if ((rc = sum_to(c, part, nb, cur_rz))) return rc;
+            k_cg_pupdate<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, nullptr, nullptr, c->cg_g, zraw, c->pc_mean, c->body_of, c->cg_p);
+            c->launches++;
+        }
     }
     double ref2 = 0.0, gg = 0.0;
     PCE_CUDA(c, cudaMemcpyAsync(&ref2, sc + 0, sizeof(double), cudaMemcpyDeviceToHost, c->st));
-    PCE_CUDA(c, cudaMemcpyAsync(&gg, sc + 2, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(&gg, sc + 1, sizeof(double), cudaMemcpyDeviceToHost, c->st));
     PCE_CUDA(c, cudaStreamSynchronize(c->st));
     const double ref = (ref2 > 0.0) ? sqrt(ref2) : 1.0;
     const double tol = c->p.tol_solver;
     int it = 0;
     inf.rel_resid = sqrt(gg) / ref;
     while (inf.rel_resid > tol && it < maxit) {
-        double* s_gg = sc + 2 + 2 * it;
-        double* s_pap = sc + 3 + 2 * it;
-        double* s_gn = sc + 2 + 2 * (it + 1);
+        double* s_pap = sc + 3 + 3 * it;
+        double* s_gn = sc + 4 + 3 * it;
+        double* next_rz = pc ? sc + 2 + 3 * (it + 1) : s_gn;
         if ((rc = op_matvec_bead(c, c->cg_p, c->cg_t))) return rc;
         inf.matvecs++;
         {
@@ -253,14 +286,21 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
             k_proj_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_t, c->cg_p, c->cg_ap, part);
             c->launches++;
             if ((rc = sum_to(c, part, nb, s_pap))) return rc;
-            k_cg_update<<<nb, BT, 0, c->st>>>(c->body_off, s_gg, s_pap, c->cg_p, c->cg_ap, c->cg_t, q, c->cg_g, c->cg_psi, part);
+            k_cg_update<<<nb, BT, 0, c->st>>>(c->body_off, cur_rz, s_pap, c->cg_p, c->cg_ap, c->cg_t, q, c->cg_g, c->cg_psi, part);
             c->launches++;
             if ((rc = sum_to(c, part, nb, s_gn))) return rc;
-            k_cg_pupdate<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, s_gg, s_gn, c->cg_g, c->cg_p);
-            c->launches++;
             PCE_CUDA(c, cudaMemcpyAsync(&gg, s_gn, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+            if (pc) {
+                if ((rc = precond_apply(c, c->cg_g, c->cg_z))) return rc;
+                k_pc_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_z, c->cg_g, c->pc_mean, part);
+                c->launches++;
+                if ((rc = sum_to(c, part, nb, next_rz))) return rc;
+            }
+            k_cg_pupdate<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, cur_rz, next_rz, c->cg_g, zraw, c->pc_mean, c->body_of, c->cg_p);
+            c->launches++;
         }
         PCE_CUDA(c, cudaStreamSynchronize(c->st));
+        cur_rz = next_rz;
         ++it;
         inf.rel_resid = sqrt(gg) / ref;
         if (!(gg == gg)) { c->err = "NaN in the Krylov residual"; return PCE_ECUDA; }

@@ -74,7 +74,9 @@ static void free_system(pce_ctx* c)
     cudaFree(c->w_kx); cudaFree(c->w_ky); cudaFree(c->w_kz);
     cudaFree(c->cg_g); cudaFree(c->cg_p); cudaFree(c->cg_t); cudaFree(c->cg_ap); cudaFree(c->cg_psi); cudaFree(c->cg_rhs);
     cudaFree(c->ev_psi); cudaFree(c->ev_ex); cudaFree(c->ev_ey); cudaFree(c->ev_ez); cudaFree(c->cg_scal);
-    cudaFree(c->hs_dev);
+    cudaFree(c->hs_dev); cudaFree(c->cg_z); cudaFree(c->pc_mean);
+    precond_free(c);
+    c->cg_z = c->pc_mean = nullptr;
     c->x = c->y = c->z = nullptr; c->body_off = c->body_of = nullptr;
     c->rx = c->ry = c->rz = c->X = c->Y = c->Z = nullptr;
     c->csr_ptr = c->csr_col = nullptr; c->csr_val = nullptr; c->nnz = c->nnz_cap = 0;
@@ -273,9 +275,11 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     ALLOC_D(c->cg_g, c->Nbead); ALLOC_D(c->cg_p, c->Nbead); ALLOC_D(c->cg_t, c->Nbead); ALLOC_D(c->cg_ap, c->Nbead);
     ALLOC_D(c->cg_psi, c->Nbead); ALLOC_D(c->cg_rhs, c->Nbead);
     ALLOC_D(c->ev_psi, N); ALLOC_D(c->ev_ex, N); ALLOC_D(c->ev_ey, N); ALLOC_D(c->ev_ez, N);
-    ALLOC_D(c->cg_scal, 2 * (c->p.max_iter + 2) + 2 + 2 * N_body + 16);
+    ALLOC_D(c->cg_scal, 3 * (c->p.max_iter + 2) + 2 + 2 * N_body + 16);
+    ALLOC_D(c->cg_z, c->Nbead); ALLOC_D(c->pc_mean, N_body);
     c->have_system = true;
     rc = positions_impl(c, x, y, z);
+    if (!rc) rc = precond_setup(c);  // needs r_ij of bodies_setup; rigid bodies: once per system
     timing_end(c);
     return rc;
 }
@@ -521,6 +525,8 @@ extern "C" int pce_get_info(const pce_ctx* c, pce_info* info)
     info->nnz_near = c->nnz;
     info->N = c->N; info->N_bead = c->Nbead; info->N_body = c->Nbody;
     info->bytes_workspace = c->bytes;
+    info->bytes_precond = c->pc_bytes;
+    info->n_precond_blocks = c->pc_on ? c->pc_nblock : 0;
     return PCE_OK;
 }
 

@@ -115,7 +115,16 @@ struct pce_ctx {
     // Krylov vectors [Nbead]
     double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr, *cg_rhs = nullptr;
     double *ev_psi = nullptr, *ev_ex = nullptr, *ev_ey = nullptr, *ev_ez = nullptr;  // [N]
-    double* cg_scal = nullptr;  // [3*(max_iter+2)]
+    double* cg_scal = nullptr;  // [3*(max_iter+2) + 2 + 2*Nbody + 16]
+    // block-Jacobi preconditioner (precond.cu)
+    bool pc_on = false;
+    float* pc_B = nullptr;            // per-body n_i x n_i fp32 blocks
+    void* pc_rows = nullptr;          // CTA -> (body, first row) map of the apply kernel
+    unsigned char* pc_has = nullptr;  // [Nbody] 1 if the body has a dense block
+    int pc_nrows_cta = 0, pc_max_n = 0, pc_nblock = 0;
+    long long pc_bytes = 0;
+    double* cg_z = nullptr;           // [Nbead] B r before the mean is removed
+    double* pc_mean = nullptr;        // [Nbody]
     // host staging for pce_step_host
     double* hs_dev = nullptr;
     size_t hs_dev_n = 0;
@@ -196,6 +205,11 @@ int bodies_setup(pce_ctx* c);
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
 int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
                double* S, double* U_body, double* U_tot, double* psi_out);
+
+// precond.cu
+int precond_setup(pce_ctx* c);
+void precond_free(pce_ctx* c);
+int precond_apply(pce_ctx* c, const double* r, double* z);
 
 // pce_api.cu
 int sum_vector(pce_ctx* c, const double* in, int n, double* out);  // deterministic two-stage sum
