@@ -181,6 +181,12 @@ int pce_step_host(pce_ctx* ctx, const double* x, const double* y, const double* 
                   double* q, double* Phi_body, double* fx, double* fy, double* fz,
                   double* F, double* T, double* S, double* U_tot, pce_solve_info* info);
 
+/* Host-only test hook (no GPU needed): the real-space pair kernel R(r) (eq. 20) and dR/dr exactly as
+ * the device evaluates them -- piecewise degree-7 polynomials in r^2 of the six exp/erfc terms plus the closed-form
+ * Heaviside term -- for n radii r[i] in [a/4, r_c); entries outside that range come back NaN (the device uses the
+ * exact formula there).  All pointers host. */
+int pce_real_kernel_host(double a, double xi, double rc, double eps_f, int n, const double* r, double* R, double* dR);
+
 int pce_set_timing(pce_ctx* ctx, int enabled);          /* per-pass CUDA events on/off (default off) */
 int pce_get_timings(const pce_ctx* ctx, pce_timings* t);
 int pce_get_info(const pce_ctx* ctx, pce_info* info);

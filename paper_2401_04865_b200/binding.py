@@ -21,7 +21,7 @@ PCE_OK, PCE_EINVAL, PCE_ENOMEM, PCE_ECUDA, PCE_ECUFFT, PCE_ENOCONV, PCE_ESTATE =
 EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
-    "pce_get_info", "pce_launch_count",
+    "pce_get_info", "pce_launch_count", "pce_real_kernel_host",
 )
 
 
@@ -87,11 +87,25 @@ def load():
     lib.pce_get_info.argtypes = [vp, C.POINTER(PceInfo)]
     lib.pce_launch_count.argtypes = [vp]
     lib.pce_launch_count.restype = C.c_longlong
+    lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
+
+
+def real_kernel_host(a, xi, rc, r, eps_f=1.0):
+    """R(r), dR/dr of eq. 20 as the device evaluates them (host-only test hook; NaN outside [a/4, rc))."""
+    lib = load()
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    R, dR = np.empty_like(r), np.empty_like(r)
+    dp = C.POINTER(C.c_double)
+    rc_ = lib.pce_real_kernel_host(float(a), float(xi), float(rc), float(eps_f), r.size, r.ctypes.data_as(dp), R.ctypes.data_as(dp),
+                                   dR.ctypes.data_as(dp))
+    if rc_ != PCE_OK:
+        raise PceError(rc_, "pce_real_kernel_host: bad arguments")
+    return R, dR
 
 
 def _d3(v):

@@ -238,8 +238,8 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
         if (info) *info = inf;
         return PCE_OK;
     }
-    // 2. potentials of the starting charges at every bead (ions included as sources): one full evaluation
-    int rc = op_evaluate(c, q, c->ev_psi, nullptr, nullptr, nullptr);
+    // 2. potentials of the starting charges at every bead (ions included as sources): all sources, bead targets
+    int rc = op_evaluate_at_beads(c, q, c->ev_psi);
     if (rc) return rc;
     inf.matvecs = 1;
     const int maxit = c->p.max_iter;

@@ -93,7 +93,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     cudaStreamSynchronize(c->st);
     free_system(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -166,7 +166,9 @@ static int create_impl(pce_ctx* c)
     cufftSetWorkArea(c->planB, c->fft_work);
     cufftSetStream(c->planF, c->st);
     cufftSetStream(c->planB, c->st);
-    return wave_bricks_init(c);
+    int rcw = wave_bricks_init(c);
+    if (rcw) return rcw;
+    return realtab_upload(c);
 }
 
 extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
@@ -355,27 +357,29 @@ __global__ void k_finalize(int n, const int* __restrict__ inv_r, const int* __re
     if (field) { ex[j] = rx[ir] + kx[iw]; ey[j] = ry[ir] + ky[iw]; ez[j] = rz[ir] + kz[iw]; }
 }
 
-// rb: real-space cells, wb: mesh tiles of the same particle subset
-static int apply_operator(pce_ctx* c, Bins& rb, Bins& wb, bool use_csr, const double* q, double* psi, double* Ex, double* Ey, double* Ez)
+// sources: the particle subset (sr: real-space cells, sw: mesh bins) whose charges q (caller order of that subset) act;
+// targets: the subset (tr, tw) where potentials / fields are wanted.  Both subsets are prefixes of the particle list.
+static int apply_operator(pce_ctx* c, Bins& sr, Bins& sw, Bins& tr, Bins& tw, bool use_csr, const double* q, double* psi, double* Ex,
+                          double* Ey, double* Ez)
 {
     const bool field = (Ex != nullptr);
-    const int n = rb.n;
+    const int n = tr.n;
     int rc;
     {
         PassTimer t(c, PASS_OTHER);
-        if ((rc = gather_by_perm(c, n, rb.perm, q, rb.qs))) return rc;
-        if ((rc = gather_by_perm(c, n, wb.perm, q, wb.qs))) return rc;
-        if ((rc = sum_vector(c, q, n, c->scal))) return rc;
+        if ((rc = gather_by_perm(c, sr.n, sr.perm, q, sr.qs))) return rc;
+        if ((rc = gather_by_perm(c, sw.n, sw.perm, q, sw.qs))) return rc;
+        if ((rc = sum_vector(c, q, sr.n, c->scal))) return rc;
     }
-    if (use_csr) rc = real_csr_spmv(c, rb, c->w_real);                                   // step 1 (cached), eq. 20-21
-    else rc = real_direct(c, rb, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);           // step 1, eq. 20-21
+    if (use_csr) rc = real_csr_spmv(c, sr, c->w_real);                                      // step 1 (cached), eq. 20-21
+    else rc = real_direct(c, tr, sr, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);          // step 1, eq. 20-21
     if (rc) return rc;
-    if ((rc = wave_spread_bricks(c, wb))) return rc;                                      // step 2, eq. 25
+    if ((rc = wave_spread_bricks(c, sw))) return rc;                                      // step 2, eq. 25
     if ((rc = wave_fft_scale_ifft(c))) return rc;                                        // steps 3-5, eq. 26
-    if ((rc = wave_gather_bricks(c, wb, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    if ((rc = wave_gather_bricks(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
     {
         PassTimer t(c, PASS_OTHER);
-        k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, rb.inv, wb.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,
+        k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, tr.inv, tw.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,
                                                    c->w_ex, c->w_ey, c->w_ez, c->w_kx, c->w_ky, c->w_kz, Ex, Ey, Ez);
         c->launches++;
     }
@@ -388,7 +392,7 @@ int op_matvec_bead(pce_ctx* c, const double* q, double* psi)
     c->tm.n_matvec_bead++;
     c->tm.n_fft_pairs++;
     c->in_bead_matvec = true;
-    int rc = apply_operator(c, c->bead, c->wbead, true, q, psi, nullptr, nullptr, nullptr);
+    int rc = apply_operator(c, c->bead, c->wbead, c->bead, c->wbead, true, q, psi, nullptr, nullptr, nullptr);
     c->in_bead_matvec = false;
     return rc;
 }
@@ -397,7 +401,15 @@ int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey
 {
     c->tm.n_eval_full++;
     c->tm.n_fft_pairs++;
-    return apply_operator(c, c->all, c->wall, false, q, psi, Ex, Ey, Ez);
+    return apply_operator(c, c->all, c->wall, c->all, c->wall, false, q, psi, Ex, Ey, Ez);
+}
+
+// potentials at the conductor beads only, from all N charges (right-hand side of eq. 13): psi has N_bead entries
+int op_evaluate_at_beads(pce_ctx* c, const double* q, double* psi)
+{
+    c->tm.n_eval_full++;
+    c->tm.n_fft_pairs++;
+    return apply_operator(c, c->all, c->wall, c->bead, c->wbead, false, q, psi, nullptr, nullptr, nullptr);
 }
 
 extern "C" int pce_matvec(pce_ctx* c, const double* q, double* psi)

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "pce.h"
+#include "realtab.h"
 
 #define PCE_PI 3.14159265358979323846
 
@@ -71,6 +72,8 @@ struct pce_ctx {
     cudaStream_t st = nullptr;
     std::string err;
     RealConst rk;
+    RealTable rt;              // real-space kernel table (device pointer), realtab.h
+    double* rt_dev = nullptr;
     WaveConst wk;
     double V = 0, eta[3], h[3];
     double kconst = 0;  // 1/(4 xi^2 V eps)
@@ -186,9 +189,13 @@ int wrap_positions(pce_ctx* c, int n, const double* xi, const double* yi, const 
 int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out);
 
 // realspace.cu
-int real_direct(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
 int real_csr_build(pce_ctx* c, const Bins& b);
 int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s);
+
+// realtab.cu
+void realtab_build_host(double a, double xi, double rc, std::vector<double>& tab, RealTable& T);
+int realtab_upload(pce_ctx* c);
 
 // wave.cu
 int wave_fft_scale_ifft(pce_ctx* c);
@@ -215,3 +222,4 @@ int precond_apply(pce_ctx* c, const double* r, double* z);
 int sum_vector(pce_ctx* c, const double* in, int n, double* out);  // deterministic two-stage sum
 int op_matvec_bead(pce_ctx* c, const double* q, double* psi);
 int op_evaluate(pce_ctx* c, const double* q, double* psi, double* Ex, double* Ey, double* Ez);
+int op_evaluate_at_beads(pce_ctx* c, const double* q, double* psi);

@@ -94,49 +94,153 @@ __device__ __forceinline__ void for_neighbors(const CellGeom& g, const int* __re
     }
 }
 
-// ---------------------------------------------------------------- direct pass
-struct OpDirect {
-    const RealConst& k;
-    const double* __restrict__ qs;
-    bool field;
-    double psi = 0, ex = 0, ey = 0, ez = 0;
-    __device__ OpDirect(const RealConst& k_, const double* q_, bool f) : k(k_), qs(q_), field(f) {}
-    __device__ __forceinline__ void operator()(int j, double dx, double dy, double dz, double r2)
-    {
-        const double q = qs[j];
-        if (r2 == 0.0) { psi += k.R0 * q; return; }  // coincident distinct particles: limit value, no field
-        const double r = sqrt(r2);
-        double R, dR;
-        pair_kernel(k, r, R, dR);
-        psi += R * q;
-        if (field) {
-            const double f = -dR * q / r;
-            ex += f * dx; ey += f * dy; ez += f * dz;
-        }
-    }
-};
-
-__global__ void __launch_bounds__(128)
-k_real_direct(int n, CellGeom g, RealConst k, const int* __restrict__ cell_start, const double* __restrict__ xs,
-              const double* __restrict__ ys, const double* __restrict__ zs, const double* __restrict__ qs, int field,
-              double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey, double* __restrict__ ez)
+// R(r) and g = -R'(r)/r (times eps_f) at s = r^2 > 0: table of realtab.h + closed-form Heaviside term; exact below s_lo
+__device__ __forceinline__ void pair_eval(const RealConst& k, const RealTable& T, double s, bool field, double& R, double& g)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    OpDirect op(k, qs, field != 0);
-    for_neighbors(g, cell_start, xs, ys, zs, i, k.rc2, op);
-    psi[i] = (op.psi + k.R0 * qs[i]) * k.inv_eps;  // + self term, eq. 21
-    if (field) {
-        ex[i] = op.ex * k.inv_eps; ey[i] = op.ey * k.inv_eps; ez[i] = op.ez * k.inv_eps;
+    if (s >= T.s_lo) {
+        rt_eval(T, s, field, R, g);
+        if (s < k.two_a * k.two_a) {  // overlapping shells: Heaviside term of eq. 20 (reading G3)
+            const double ir = rsqrt(s), r = s * ir, m = r - k.two_a;
+            R -= m * m * k.t_lin * ir;                                      // t_lin = 1/(16 pi a^2)
+            g -= (0.25 / PCE_PI * ir * ir - k.t_lin) * ir;
+        }
+    } else {
+        const double r = sqrt(s);
+        double dR;
+        pair_kernel(k, r, R, dR);
+        g = -dR / r;
     }
 }
 
-int real_direct(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s)
+// ---------------------------------------------------------------- direct pass (step 1)
+// The paper runs one thread per particle over the neighbour cells.  Here one WARP owns a target cell: lane l owns
+// target l of a chunk of 32, the sources of each of the 27 neighbour cells (or periodic images, reading A10) are
+// staged 64 at a time in the warp's shared memory by coalesced loads, every lane tests its target against the 64
+// staged sources (broadcast reads, 7 fp64 instructions per test) and records the hits in a 64-bit mask; the kernel
+// (two degree-7 polynomials from the table) is then evaluated hit by hit, so the expensive body runs max_lane(hits)
+// times per stage instead of once per candidate.  Targets and sources may be different subsets with the same cell
+// geometry (targets = beads, sources = all, for the right-hand side of eq. 13).  A source at r = 0 -- the target
+// itself (the beta = alpha, n = 0 term) or a coincident particle (reading A9) -- contributes R(0) q (eq. 21) and no field.
+constexpr int RS_WARPS = 4;
+constexpr int RS_STAGE = 64;
+
+template <bool FIELD>
+__global__ void __launch_bounds__(RS_WARPS * 32)
+k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_start, const double* __restrict__ txs,
+             const double* __restrict__ tys, const double* __restrict__ tzs, const int* __restrict__ s_start,
+             const double* __restrict__ sxs, const double* __restrict__ sys, const double* __restrict__ szs,
+             const double* __restrict__ sqs, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
+             double* __restrict__ ez, int* __restrict__ work_ctr)
 {
-    if (b.n == 0) return PCE_OK;
+    __shared__ double2 sh_xy[RS_WARPS][RS_STAGE];
+    __shared__ double2 sh_zq[RS_WARPS][RS_STAGE];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double2* sxy = sh_xy[warp];
+    double2* szq = sh_zq[warp];
+    const int ncell = g.nc[0] * g.nc[1] * g.nc[2];
+    for (;;) {
+        int cell = 0;
+        if (lane == 0) cell = atomicAdd(work_ctr, 1);
+        cell = __shfl_sync(0xffffffffu, cell, 0);
+        if (cell >= ncell) return;
+        const int tb = t_start[cell], te = t_start[cell + 1];
+        if (te == tb) continue;
+        const int cx = cell % g.nc[0], cy = (cell / g.nc[0]) % g.nc[1], cz = cell / (g.nc[0] * g.nc[1]);
+        for (int t0 = tb; t0 < te; t0 += 32) {
+            const int i = t0 + lane;
+            const bool valid = i < te;
+            const double xi = valid ? txs[i] : 1e150, yi = valid ? tys[i] : 1e150, zi = valid ? tzs[i] : 1e150;
+            double a_psi = 0.0, a_x = 0.0, a_y = 0.0, a_z = 0.0;
+            for (int oz = -g.range[2]; oz <= g.range[2]; ++oz) {
+                int nz = cz + oz;
+                const int wz = floor_div(nz, g.nc[2]);
+                nz -= wz * g.nc[2];
+                const double shz = wz * g.L[2];
+                for (int oy = -g.range[1]; oy <= g.range[1]; ++oy) {
+                    int ny = cy + oy;
+                    const int wy = floor_div(ny, g.nc[1]);
+                    ny -= wy * g.nc[1];
+                    const double shy = wy * g.L[1];
+                    for (int ox = -g.range[0]; ox <= g.range[0]; ++ox) {
+                        int nx = cx + ox;
+                        const int wx = floor_div(nx, g.nc[0]);
+                        nx -= wx * g.nc[0];
+                        const double shx = wx * g.L[0];
+                        const int scell = (nz * g.nc[1] + ny) * g.nc[0] + nx;
+                        const int jb = s_start[scell], je = s_start[scell + 1];
+                        for (int j0 = jb; j0 < je; j0 += RS_STAGE) {
+                            const int cnt = min(RS_STAGE, je - j0);
+                            __syncwarp();
+#pragma unroll
+                            for (int h = 0; h < RS_STAGE / 32; ++h) {
+                                const int jj = lane + 32 * h;
+                                if (jj < cnt) {
+                                    const int j = j0 + jj;
+                                    sxy[jj] = make_double2(sxs[j] + shx, sys[j] + shy);
+                                    szq[jj] = make_double2(szs[j] + shz, sqs[j]);
+                                }
+                            }
+                            __syncwarp();
+                            unsigned long long mask = 0ull;
+#pragma unroll 4
+                            for (int jj = 0; jj < cnt; ++jj) {
+                                const double2 pxy = sxy[jj];
+                                const double pz = szq[jj].x;
+                                const double dx = xi - pxy.x, dy = yi - pxy.y, dz = zi - pz;
+                                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                                if (r2 < k.rc2) mask |= 1ull << jj;
+                            }
+                            while (mask) {
+                                const int jj = __ffsll((long long)mask) - 1;
+                                mask &= mask - 1ull;
+                                const double2 pxy = sxy[jj], pzq = szq[jj];
+                                const double dx = xi - pxy.x, dy = yi - pxy.y, dz = zi - pzq.x;
+                                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                                if (r2 == 0.0) { a_psi = fma(k.R0, pzq.y, a_psi); continue; }  // eq. 21
+                                double R, gk = 0.0;
+                                pair_eval(k, T, r2, FIELD, R, gk);
+                                a_psi = fma(R, pzq.y, a_psi);
+                                if (FIELD) {
+                                    const double f = gk * pzq.y;
+                                    a_x = fma(f, dx, a_x); a_y = fma(f, dy, a_y); a_z = fma(f, dz, a_z);
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+            if (valid) {
+                psi[i] = a_psi * k.inv_eps;
+                if (FIELD) { ex[i] = a_x * k.inv_eps; ey[i] = a_y * k.inv_eps; ez[i] = a_z * k.inv_eps; }
+            }
+        }
+    }
+}
+
+// potentials (and fields) at the particles of tb from the charges sb.qs of the particles of sb (same cell geometry)
+int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s)
+{
+    if (tb.n == 0) return PCE_OK;
     PassTimer t(c, PASS_REAL);
-    k_real_direct<<<cdiv(b.n, 128), 128, 0, c->st>>>(b.n, geom_of(b), c->rk, b.cell_start, b.xs, b.ys, b.zs, b.qs, field ? 1 : 0,
-                                                     psi_s, ex_s, ey_s, ez_s);
+    if (sb.n == 0) {
+        PCE_CUDA(c, cudaMemsetAsync(psi_s, 0, (size_t)tb.n * sizeof(double), c->st));
+        if (field) {
+            PCE_CUDA(c, cudaMemsetAsync(ex_s, 0, (size_t)tb.n * sizeof(double), c->st));
+            PCE_CUDA(c, cudaMemsetAsync(ey_s, 0, (size_t)tb.n * sizeof(double), c->st));
+            PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)tb.n * sizeof(double), c->st));
+        }
+        return PCE_OK;
+    }
+    PCE_CUDA(c, cudaMemsetAsync(c->work_ctr + 1, 0, sizeof(int), c->st));
+    int blocks = c->num_sm * 8;
+    const int need = cdiv(tb.ncell, RS_WARPS);
+    if (blocks > need) blocks = need;
+    if (field)
+        k_real_cells<true><<<blocks, RS_WARPS * 32, 0, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+                                                                 sb.xs, sb.ys, sb.zs, sb.qs, psi_s, ex_s, ey_s, ez_s, c->work_ctr + 1);
+    else
+        k_real_cells<false><<<blocks, RS_WARPS * 32, 0, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+                                                                  sb.xs, sb.ys, sb.zs, sb.qs, psi_s, nullptr, nullptr, nullptr, c->work_ctr + 1);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -161,14 +265,15 @@ k_csr_count(int n, CellGeom g, double rc2, const int* __restrict__ cell_start, c
 
 struct OpFill {
     const RealConst& k;
+    const RealTable& T;
     int* __restrict__ col;
     double* __restrict__ val;
     long long pos;
-    __device__ OpFill(const RealConst& k_, int* c_, double* v_, long long p_) : k(k_), col(c_), val(v_), pos(p_) {}
+    __device__ OpFill(const RealConst& k_, const RealTable& T_, int* c_, double* v_, long long p_) : k(k_), T(T_), col(c_), val(v_), pos(p_) {}
     __device__ __forceinline__ void operator()(int j, double, double, double, double r2)
     {
-        double R = k.R0, dR;
-        if (r2 > 0.0) pair_kernel(k, sqrt(r2), R, dR);
+        double R = k.R0, gk;
+        if (r2 > 0.0) pair_eval(k, T, r2, false, R, gk);
         col[pos] = j;
         val[pos] = R * k.inv_eps;
         ++pos;
@@ -176,7 +281,7 @@ struct OpFill {
 };
 
 __global__ void __launch_bounds__(128)
-k_csr_fill(int n, CellGeom g, RealConst k, const int* __restrict__ cell_start, const double* __restrict__ xs,
+k_csr_fill(int n, CellGeom g, RealConst k, RealTable T, const int* __restrict__ cell_start, const double* __restrict__ xs,
            const double* __restrict__ ys, const double* __restrict__ zs, const int* __restrict__ row_ptr,
            int* __restrict__ col, double* __restrict__ val)
 {
@@ -185,7 +290,7 @@ k_csr_fill(int n, CellGeom g, RealConst k, const int* __restrict__ cell_start, c
     long long pos = row_ptr[i];
     col[pos] = i;
     val[pos] = k.R0 * k.inv_eps;  // self term, eq. 21
-    OpFill op(k, col, val, pos + 1);
+    OpFill op(k, T, col, val, pos + 1);
     for_neighbors(g, cell_start, xs, ys, zs, i, k.rc2, op);
 }
 
@@ -218,7 +323,7 @@ int real_csr_build(pce_ctx* c, const Bins& b)
         c->bytes += c->nnz_cap * 12;
     }
     c->nnz = nnz;
-    k_csr_fill<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr, c->csr_col,
+    k_csr_fill<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr, c->csr_col,
                                                 c->csr_val);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
