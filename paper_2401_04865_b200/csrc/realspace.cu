@@ -130,10 +130,17 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
              const double* __restrict__ tys, const double* __restrict__ tzs, const int* __restrict__ s_start,
              const double* __restrict__ sxs, const double* __restrict__ sys, const double* __restrict__ szs,
              const double* __restrict__ sqs, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
-             double* __restrict__ ez, int* __restrict__ work_ctr)
+             double* __restrict__ ez, int* __restrict__ work_ctr, int tab_in_smem)
 {
     __shared__ double2 sh_xy[RS_WARPS][RS_STAGE];
     __shared__ double2 sh_zq[RS_WARPS][RS_STAGE];
+    extern __shared__ double sh_tab[];  // copy of the kernel table (potential rows, with FIELD also the field rows)
+    if (tab_in_smem) {
+        const int nt = (FIELD ? RT_STRIDE : RT_DEG + 1) * T.n_int;
+        for (int e = threadIdx.x; e < nt; e += blockDim.x) sh_tab[e] = T.tab[e];
+        __syncthreads();
+        T.tab = sh_tab;
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double2* sxy = sh_xy[warp];
     double2* szq = sh_zq[warp];
@@ -232,15 +239,22 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
         return PCE_OK;
     }
     PCE_CUDA(c, cudaMemsetAsync(c->work_ctr + 1, 0, sizeof(int), c->st));
-    int blocks = c->num_sm * 8;
+    const size_t tab_bytes = (size_t)(field ? RT_STRIDE : RT_DEG + 1) * c->rt.n_int * sizeof(double);
+    const int in_smem = tab_bytes <= 96 * 1024 ? 1 : 0;  // else the table is read from global memory (L1/L2)
+    const size_t dyn = in_smem ? tab_bytes : 0;
+    const int per_sm = in_smem ? (int)((200 * 1024) / (dyn + 8192 + 1024)) : 8;
+    int blocks = c->num_sm * (per_sm < 1 ? 1 : per_sm > 8 ? 8 : per_sm);
     const int need = cdiv(tb.ncell, RS_WARPS);
     if (blocks > need) blocks = need;
-    if (field)
-        k_real_cells<true><<<blocks, RS_WARPS * 32, 0, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
-                                                                 sb.xs, sb.ys, sb.zs, sb.qs, psi_s, ex_s, ey_s, ez_s, c->work_ctr + 1);
-    else
-        k_real_cells<false><<<blocks, RS_WARPS * 32, 0, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
-                                                                  sb.xs, sb.ys, sb.zs, sb.qs, psi_s, nullptr, nullptr, nullptr, c->work_ctr + 1);
+    if (field) {
+        if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        k_real_cells<true><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+                                                                   sb.xs, sb.ys, sb.zs, sb.qs, psi_s, ex_s, ey_s, ez_s, c->work_ctr + 1, in_smem);
+    } else {
+        if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+        k_real_cells<false><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+                                                                    sb.xs, sb.ys, sb.zs, sb.qs, psi_s, nullptr, nullptr, nullptr, c->work_ctr + 1, in_smem);
+    }
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -283,8 +297,15 @@ struct OpFill {
 __global__ void __launch_bounds__(128)
 k_csr_fill(int n, CellGeom g, RealConst k, RealTable T, const int* __restrict__ cell_start, const double* __restrict__ xs,
            const double* __restrict__ ys, const double* __restrict__ zs, const int* __restrict__ row_ptr,
-           int* __restrict__ col, double* __restrict__ val)
+           int* __restrict__ col, double* __restrict__ val, int tab_in_smem)
 {
+    extern __shared__ double sh_tab[];
+    if (tab_in_smem) {
+        const int nt = (RT_DEG + 1) * T.n_int;
+        for (int e = threadIdx.x; e < nt; e += blockDim.x) sh_tab[e] = T.tab[e];
+        __syncthreads();
+        T.tab = sh_tab;
+    }
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     long long pos = row_ptr[i];
@@ -323,8 +344,11 @@ int real_csr_build(pce_ctx* c, const Bins& b)
         c->bytes += c->nnz_cap * 12;
     }
     c->nnz = nnz;
-    k_csr_fill<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr, c->csr_col,
-                                                c->csr_val);
+    const size_t tab_bytes = (size_t)(RT_DEG + 1) * c->rt.n_int * sizeof(double);
+    const int in_smem = tab_bytes <= 96 * 1024 ? 1 : 0;
+    if (in_smem && tab_bytes > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_csr_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_bytes));
+    k_csr_fill<<<cdiv(n, 128), 128, in_smem ? tab_bytes : 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr,
+                                                                      c->csr_col, c->csr_val, in_smem);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;

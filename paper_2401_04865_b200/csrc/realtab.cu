@@ -92,8 +92,13 @@ void realtab_build_host(double a, double xi, double rc, std::vector<double>& tab
             const long double s = s0 + 0.5L * (t + 1.0L) * w;
             N_gN(k, sqrtl(s), fN[j], fg[j]);
         }
-        cheb_fit(fN, &tab[(size_t)i * RT_STRIDE]);
-        cheb_fit(fg, &tab[(size_t)i * RT_STRIDE + n]);
+        double cN[n], cg[n];
+        cheb_fit(fN, cN);
+        cheb_fit(fg, cg);
+        for (int kk = 0; kk < n; ++kk) {
+            tab[(size_t)kk * T.n_int + i] = cN[kk];
+            tab[(size_t)(n + kk) * T.n_int + i] = cg[kk];
+        }
     }
     T.tab = tab.data();
 }

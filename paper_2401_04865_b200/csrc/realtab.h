@@ -16,7 +16,9 @@ constexpr int RT_DEG = 7;                // polynomial degree
 constexpr int RT_STRIDE = 2 * (RT_DEG + 1);  // doubles per interval: N coefficients, then g_N coefficients
 
 struct RealTable {
-    const double* tab = nullptr;  // [n_int][RT_STRIDE] (device pointer in kernels, host pointer in the test hook)
+    // [RT_STRIDE][n_int], coefficient-major: lanes that look up different intervals touch consecutive words, so a
+    // copy in shared memory is read with few bank conflicts.  Rows 0..RT_DEG: N; rows RT_DEG+1..: g_N.
+    const double* tab = nullptr;  // device pointer (global or shared) in kernels, host pointer in the test hook
     int key_lo = 0, n_int = 0;    // key(s) = hi32(s) >> (20 - RT_BITS); interval = key - key_lo
     double s_lo = 0.0;            // first tabulated s
 };
@@ -54,16 +56,17 @@ RT_HD void rt_eval(const RealTable& T, double s, bool field, double& N, double& 
     // 2 / width: width = 2^(e - 1023 - RT_BITS) with e = key >> RT_BITS  ->  exponent field 1023 + 1 + RT_BITS - (e - 1023)
     const double two_inv_w = rt_from_hi((2047 + RT_BITS - (key >> RT_BITS)) << 20);
     const double t = (s - s0) * two_inv_w - 1.0;
-    const double* c = T.tab + (size_t)(key - T.key_lo) * RT_STRIDE;
-    double p = c[RT_DEG];
+    const int n = T.n_int;
+    const double* c = T.tab + (key - T.key_lo);
+    double p = c[RT_DEG * n];
 #pragma unroll
-    for (int k = RT_DEG - 1; k >= 0; --k) p = p * t + c[k];
+    for (int k = RT_DEG - 1; k >= 0; --k) p = p * t + c[k * n];
     N = p;
     if (field) {
-        const double* d = c + RT_DEG + 1;
-        double q = d[RT_DEG];
+        const double* d = c + (RT_DEG + 1) * n;
+        double q = d[RT_DEG * n];
 #pragma unroll
-        for (int k = RT_DEG - 1; k >= 0; --k) q = q * t + d[k];
+        for (int k = RT_DEG - 1; k >= 0; --k) q = q * t + d[k * n];
         g = q;
     }
 }
