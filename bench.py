@@ -179,6 +179,20 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+# ---------------------------------------------------------------- replicas (multi-GPU: no sharding)
+def reduce_over_ranks(dist, ms, count, device):
+    """Whole-job figures of N independent replicas: (max over ranks of the timed ms, sum over ranks of the count).
+    `dist` is an initialised torch.distributed module (nccl on GPUs; gloo in the CPU tests) or None for one rank."""
+    if dist is None:
+        return float(ms), float(count)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([count], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(c.item())
+
+
 # ---------------------------------------------------------------- our arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -247,15 +261,7 @@ def run_ours(args, rank, world, local_rank):
     ctx.set_timing(False)
     total_ms = float(sum(ms_steps))
     n_apply = n_m1 + n_m2
-    if dist:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        cnt = torch.tensor([n_apply], dtype=torch.float64, device="cuda")
-        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
-        n_apply_all = float(cnt.item())
-    else:
-        n_apply_all = float(n_apply)
+    total_ms, n_apply_all = reduce_over_ranks(dist, total_ms, n_apply, "cuda")
     value = n_apply_all / (total_ms * 1e-3)
 
     # ---- end to end through the host-buffer call (H2D + D2H inside the timed region)
@@ -283,13 +289,7 @@ def run_ours(args, rank, world, local_rank):
         ev1.record()
         torch.cuda.synchronize()
         ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))  # the call is synchronous: host clock bounds it
-        if dist:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-            cnt = torch.tensor([n_e2e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
-            n_e2e = float(cnt.item())
+        ms, n_e2e = reduce_over_ranks(dist, ms, n_e2e, "cuda")
         e2e = {"value": n_e2e / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * (3 * w.N + nb + w.N_ion),
                "d2h_bytes_per_step": 8 * (w.N + nb + 3 * w.N + 9 * nb + 3), "ms_per_step": ms / args.steps}
     if rank != 0:
