@@ -323,7 +323,10 @@ def run_ours(args, rank, world, local_rank):
     roof = dict(own[dom])
     roof["kernel"] = dom
     roof["peak_source"] = peak_src
-    roof["traffic"] = None  # dram bytes from ncu: see profiles/
+    roof["traffic"] = None  # dram bytes per launch from the committed ncu --set full capture (config 5 only)
+    tpath = os.path.join(ROOT, "profiles", "r1d_traffic.json")
+    if args.config == 5 and os.path.exists(tpath):
+        roof["traffic"] = json.load(open(tpath)).get(dom)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
