@@ -18,7 +18,10 @@
 //      started from per-particle coefficients of k_window_coef (phi = -s0 mod 8,
 //      e1 = exp(-2 aw u0), c0 = exp(-aw u0^2) e1^phi, e8 = e1^8):
 //      W(phi + 8m) = c0 e8^m exp(-aw (phi + 8m)^2), t(r) = e1 exp(-aw (2r + 1)); no exp here;
-//   4. accumulate: per hit every lane issues 5 shared-memory loads, 4 DMUL and 16 DFMA.
+//   4. accumulate on the fp64 tensor path (mma.sync m8n8k4.f64, measured 37.1 TFLOP/s against 33.3 for DFMA chains):
+//      per brick the spread is the contraction H_z[y][x] = sum_h (wy_h[y] q_h wz_h[z]) wx_h[x] over the hits h of
+//      the brick, the gather T_z[h][x] = sum_y wy_h[y] H~_z[y][x]; see the kernels.  The (x, y) patch per lane of
+//      the description above becomes the mma fragment layout: lane l holds (y = l/4, x = 2(l%4), 2(l%4)+1) of all 8 planes.
 // Spread writes every mesh point exactly once (no atomics, no memset, deterministic).
 // Gather keeps the brick of H~ in registers, reduces the 32 lane partials of 8 hits (4 with
 // the field) at a time by a transposing butterfly and issues one global fp64 atomicAdd per
@@ -259,7 +262,18 @@ k_window_coef(int n, WaveConst wc, const double* __restrict__ xs, const double* 
     }                                                                                                                   \
     __syncwarp();
 
+// ---------------------------------------------------------------- fp64 tensor-core step
+// D(8x8) += A(8x4) B(4x8), fp64 (mma.sync m8n8k4; tcgen05 has no fp64 kind).  With g = lane/4, t = lane%4 a lane holds
+// A[g][t], B[t][g] and the pair D[g][2t], D[g][2t+1].
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
 // ---------------------------------------------------------------- spread
+// Per brick and mesh plane z the spread is a dense contraction over the hits h of the brick:
+//     H_z[y][x] = sum_h (wy_h[y] q_h wz_h[z]) wx_h[x]  =  (A_z B)[y][x],  A_z = 8 x hits, B = hits x 8,
+// issued four hits at a time as one fp64 mma per plane: 8 DMUL + 8 DMMA per 4 hits instead of 16 DMUL + 64 DFMA.
 __global__ void __launch_bounds__(BWARPS * 32, 5)
 k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
@@ -272,34 +286,32 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE_PSI>& s = sm[warp];
-    const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    const int g = lane >> 2, t = lane & 3;  // mma fragment coordinates
     for (;;) {  // persistent warps: bricks are handed out by a global counter
     int brick_id = 0;
     if (lane == 0) brick_id = atomicAdd(work_ctr, 1);
     brick_id = __shfl_sync(0xffffffffu, brick_id, 0);
     Brick br;
     if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, brick_id)) return;
-    double acc[4][4];
+    double acc[BR][2];  // plane z: H[z][y = g][x = 2t, 2t + 1]
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) acc[j][i] = 0.0;
+    for (int z = 0; z < BR; ++z) { acc[z][0] = 0.0; acc[z][1] = 0.0; }
 
 #define SPREAD_PROCESS(NH)                                                                                              \
     {                                                                                                                   \
         const int nh = (NH);                                                                                            \
         BRICK_WEIGHTS(false, STRIDE_PSI, BR, qs[p])                                                                     \
-        for (int slot = 0; slot < nh; ++slot) {                                                                         \
-            const double* w = s.wt + slot * STRIDE_PSI;                                                                 \
-            const double2 x01 = *reinterpret_cast<const double2*>(w + px);                                              \
-            const double2 x23 = *reinterpret_cast<const double2*>(w + px + 2);                                          \
-            const double2 y01 = *reinterpret_cast<const double2*>(w + BR + py);                                         \
-            const double2 y23 = *reinterpret_cast<const double2*>(w + BR + py + 2);                                     \
-            const double wzq = w[2 * BR + pz];                                                                          \
-            const double cy[4] = {wzq * y01.x, wzq * y01.y, wzq * y23.x, wzq * y23.y};                                  \
-            const double wx[4] = {x01.x, x01.y, x23.x, x23.y};                                                          \
-            _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                               \
-                _Pragma("unroll") for (int i = 0; i < 4; ++i) acc[j][i] = fma(cy[j], wx[i], acc[j][i]);                 \
+        for (int sb = 0; sb < nh; sb += 4) {                                                                            \
+            const bool live = sb + t < nh;                                                                              \
+            const double* w = s.wt + (sb + t) * STRIDE_PSI;                                                             \
+            const double bx = live ? w[g] : 0.0;                      /* B[t][g] = wx_h[x = g]            */            \
+            const double ay = live ? w[BR + g] : 0.0;                 /* wy_h[y = g]                      */            \
+            double wz[BR];                                            /* q_h wz_h[0..7]                   */            \
+            _Pragma("unroll") for (int z = 0; z < BR; z += 2) {                                                         \
+                const double2 v = *reinterpret_cast<const double2*>(w + 2 * BR + z);                                    \
+                wz[z] = v.x; wz[z + 1] = v.y;                                                                           \
+            }                                                                                                           \
+            _Pragma("unroll") for (int z = 0; z < BR; ++z) dmma884(acc[z][0], acc[z][1], ay * wz[z], bx);               \
         }                                                                                                               \
         __syncwarp();                                                                                                   \
     }
@@ -307,51 +319,30 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     BRICK_WALK(SPREAD_PROCESS)
 #undef SPREAD_PROCESS
 
-    const int gz = br.b0[2] + pz;
     const size_t Nx = wc.Ng[0], Ny = wc.Ng[1];
-    const int gx = br.b0[0] + px;
+    const int gx = br.b0[0] + 2 * t, gy = br.b0[1] + g;
+    if (gy < wc.Ng[1]) {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const int gy = br.b0[1] + py + j;
-        if (gz >= wc.Ng[2] || gy >= wc.Ng[1]) break;
-        double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
-        if (vec_ok && gx + 3 < wc.Ng[0]) {
-            *reinterpret_cast<double2*>(row) = make_double2(acc[j][0], acc[j][1]);
-            *reinterpret_cast<double2*>(row + 2) = make_double2(acc[j][2], acc[j][3]);
-        } else {
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (gx + i < wc.Ng[0]) row[i] = acc[j][i];
+        for (int z = 0; z < BR; ++z) {
+            const int gz = br.b0[2] + z;
+            if (gz >= wc.Ng[2]) break;
+            double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
+            if (vec_ok && gx + 1 < wc.Ng[0]) {
+                *reinterpret_cast<double2*>(row) = make_double2(acc[z][0], acc[z][1]);
+            } else {
+                if (gx < wc.Ng[0]) row[0] = acc[z][0];
+                if (gx + 1 < wc.Ng[0]) row[1] = acc[z][1];
+            }
         }
     }
     __syncwarp();
     }  // next brick
 }
 // ---------------------------------------------------------------- gather
-// reduce NV values per lane across the warp; afterwards lanes with (lane & (32/NV - 1)) == 0 hold the warp
-// total of value number `id`
-template <int NV>
-__device__ __forceinline__ double transpose_reduce(double (&v)[NV], int lane, int& id)
-{
-    id = 0;
-    int x = 16;
-#pragma unroll
-    for (int half = NV / 2; half >= 1; half >>= 1) {
-        const bool up = (lane & x) != 0;
-#pragma unroll
-        for (int k = 0; k < half; ++k) {
-            const double send = up ? v[k] : v[k + half];
-            const double keep = up ? v[k + half] : v[k];
-            v[k] = keep + __shfl_xor_sync(0xffffffffu, send, x);
-        }
-        if (up) id += half;
-        x >>= 1;
-    }
-    double r = v[0];
-    for (; x >= 1; x >>= 1) r += __shfl_xor_sync(0xffffffffu, r, x);
-    return r;
-}
-
+// Per brick, plane z and group of 8 hits the gather is the contraction  T_z[h][x] = sum_y wy_h[y] H~_z[y][x]  (two fp64
+// mma k-steps, the brick of H~ being the B operand held in registers), followed by  U[h][x] += wz_h[z] T_z[h][x]  and, after
+// the 8 planes,  psi_h += sum_x wx_h[x] U[h][x]  (4-lane shuffle, one atomicAdd per hit and quantity).  With the field the
+// window-gradient sums (reading A3) reuse T_z with wz u_z and wx u_x, and need a second contraction with wy u_y.
 template <bool FIELD>
 __global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 5)
 k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
@@ -361,8 +352,6 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 {
     constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
     constexpr int DW = FIELD ? 2 * BR : BR;  // doubles per dimension in the weight table
-    constexpr int G = FIELD ? 4 : 8;         // hits per butterfly
-    constexpr int NQ = FIELD ? 4 : 1;        // quantities per hit: psi (, Ex, Ey, Ez)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* tab = reinterpret_cast<double*>(smem_raw);
     WarpSmem<STRIDE>* sm = reinterpret_cast<WarpSmem<STRIDE>*>(smem_raw + NTAB * sizeof(double));
@@ -370,7 +359,8 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     const bool generic = generic_ != 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem<STRIDE>& s = sm[warp];
-    const int px = (lane & 1) * 4, py = ((lane >> 1) & 1) * 4, pz = lane >> 2;
+    const int g = lane >> 2, t = lane & 3;  // mma fragment coordinates
+    (void)vec_ok;
     for (;;) {  // persistent warps: bricks are handed out by a global counter
     int brick_id = 0;
     if (lane == 0) brick_id = atomicAdd(work_ctr, 1);
@@ -378,22 +368,19 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     Brick br;
     if (!brick_setup(wc, nbx, nby, nbz, cell_start, s, br, lane, brick_id)) return;
     if (br.M == 0) continue;
-    // the lane's 4x4 patch of H~ in registers (0 outside the mesh)
-    double H[4][4];
+    // B operands: H[z][0] = H~[z][y = t][x = g], H[z][1] = H~[z][y = t + 4][x = g]  (0 outside the mesh)
+    double H[BR][2];
     {
         const size_t Nx = wc.Ng[0], Ny = wc.Ng[1];
-        const int gz = br.b0[2] + pz, gx = br.b0[0] + px;
+        const int gx = br.b0[0] + g;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int gy = br.b0[1] + py + j;
-            const bool rowok = gz < wc.Ng[2] && gy < wc.Ng[1];
-            const double* row = grid + ((size_t)gz * Ny + gy) * Nx + gx;
-            if (rowok && vec_ok && gx + 3 < wc.Ng[0]) {
-                const double2 a = *reinterpret_cast<const double2*>(row), b = *reinterpret_cast<const double2*>(row + 2);
-                H[j][0] = a.x; H[j][1] = a.y; H[j][2] = b.x; H[j][3] = b.y;
-            } else {
+        for (int z = 0; z < BR; ++z) {
+            const int gz = br.b0[2] + z;
 #pragma unroll
-                for (int i = 0; i < 4; ++i) H[j][i] = (rowok && gx + i < wc.Ng[0]) ? row[i] : 0.0;
+            for (int k = 0; k < 2; ++k) {
+                const int gy = br.b0[1] + t + 4 * k;
+                const bool ok = gz < wc.Ng[2] && gy < wc.Ng[1] && gx < wc.Ng[0];
+                H[z][k] = ok ? grid[((size_t)gz * Ny + gy) * Nx + gx] : 0.0;
             }
         }
     }
@@ -402,55 +389,64 @@ k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
     {                                                                                                                   \
         const int nh = (NH);                                                                                            \
         BRICK_WEIGHTS(FIELD, STRIDE, DW, 1.0)                                                                           \
-        for (int sb = 0; sb < nh; sb += G) {                                                                            \
-            double v[NQ * G];                                                                                           \
-            _Pragma("unroll") for (int g = 0; g < G; ++g) {                                                             \
-                if (sb + g < nh) {                                                                                      \
-                    const double* w = s.wt + (sb + g) * STRIDE;                                                         \
-                    const double2 x01 = *reinterpret_cast<const double2*>(w + px);                                      \
-                    const double2 x23 = *reinterpret_cast<const double2*>(w + px + 2);                                  \
-                    const double2 y01 = *reinterpret_cast<const double2*>(w + DW + py);                                 \
-                    const double2 y23 = *reinterpret_cast<const double2*>(w + DW + py + 2);                             \
-                    const double wz = w[2 * DW + pz];                                                                   \
-                    const double wx[4] = {x01.x, x01.y, x23.x, x23.y};                                                  \
-                    const double wy[4] = {y01.x, y01.y, y23.x, y23.y};                                                  \
-                    double t0[4];                                                                                       \
-                    _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                       \
-                        t0[j] = fma(H[j][3], wx[3], fma(H[j][2], wx[2], fma(H[j][1], wx[1], H[j][0] * wx[0])));         \
-                    const double s0 = fma(wy[3], t0[3], fma(wy[2], t0[2], fma(wy[1], t0[1], wy[0] * t0[0])));           \
-                    if (!FIELD) {                                                                                       \
-                        v[g] = wz * s0;                                                                                 \
-                    } else {                                                                                            \
-                        const double2 xu01 = *reinterpret_cast<const double2*>(w + BR + px);                            \
-                        const double2 xu23 = *reinterpret_cast<const double2*>(w + BR + px + 2);                        \
-                        const double2 yu01 = *reinterpret_cast<const double2*>(w + DW + BR + py);                       \
-                        const double2 yu23 = *reinterpret_cast<const double2*>(w + DW + BR + py + 2);                   \
-                        const double wzu = w[2 * DW + BR + pz];                                                         \
-                        const double wxu[4] = {xu01.x, xu01.y, xu23.x, xu23.y};                                         \
-                        const double wyu[4] = {yu01.x, yu01.y, yu23.x, yu23.y};                                         \
-                        double t1[4];                                                                                   \
-                        _Pragma("unroll") for (int j = 0; j < 4; ++j)                                                   \
-                            t1[j] = fma(H[j][3], wxu[3], fma(H[j][2], wxu[2], fma(H[j][1], wxu[1], H[j][0] * wxu[0]))); \
-                        const double sx = fma(wy[3], t1[3], fma(wy[2], t1[2], fma(wy[1], t1[1], wy[0] * t1[0])));       \
-                        const double sy = fma(wyu[3], t0[3], fma(wyu[2], t0[2], fma(wyu[1], t0[1], wyu[0] * t0[0])));   \
-                        v[NQ * g + 0] = wz * s0;                                                                        \
-                        v[NQ * g + 1] = wz * sx;                                                                        \
-                        v[NQ * g + 2] = wz * sy;                                                                        \
-                        v[NQ * g + 3] = wzu * s0;                                                                       \
-                    }                                                                                                   \
-                } else {                                                                                                \
-                    _Pragma("unroll") for (int k = 0; k < NQ; ++k) v[NQ * g + k] = 0.0;                                 \
-                }                                                                                                       \
+        for (int sb = 0; sb < nh; sb += 8) {                                                                            \
+            const int hr = sb + g;                                                                                      \
+            const bool live = hr < nh;                                                                                  \
+            const double* w = s.wt + (live ? hr : 0) * STRIDE;                                                          \
+            const double a0 = live ? w[DW + t] : 0.0, a1 = live ? w[DW + t + 4] : 0.0;          /* wy_h[y]    */        \
+            const double2 wx2 = *reinterpret_cast<const double2*>(w + 2 * t);                   /* wx_h[2t..] */        \
+            double wz[BR];                                                                                              \
+            _Pragma("unroll") for (int z = 0; z < BR; z += 2) {                                                         \
+                const double2 v = *reinterpret_cast<const double2*>(w + 2 * DW + z);                                    \
+                wz[z] = v.x; wz[z + 1] = v.y;                                                                           \
             }                                                                                                           \
-            int id;                                                                                                     \
-            const double r = transpose_reduce<NQ * G>(v, lane, id);                                                     \
-            const int g = id / NQ, qn = id - g * NQ;                                                                    \
-            if ((lane & (32 / (NQ * G) - 1)) == 0 && sb + g < nh) {                                                     \
-                const int p = s.qidx[sb + g];                                                                           \
-                if (qn == 0) atomicAdd(&psi[p], r);                                                                     \
-                else if (qn == 1) atomicAdd(&ex[p], -wc.grad_fac[0] * r); /* E = -grad_a, dW/dx_a = +grad_fac u W */    \
-                else if (qn == 2) atomicAdd(&ey[p], -wc.grad_fac[1] * r);                                               \
-                else atomicAdd(&ez[p], -wc.grad_fac[2] * r);                                                            \
+            if (!FIELD) {                                                                                               \
+                double u0 = 0.0, u1 = 0.0;                                                                              \
+                _Pragma("unroll") for (int z = 0; z < BR; ++z) {                                                        \
+                    double t0 = 0.0, t1 = 0.0;                                                                          \
+                    dmma884(t0, t1, a0, H[z][0]);                                                                       \
+                    dmma884(t0, t1, a1, H[z][1]);                                                                       \
+                    u0 = fma(wz[z], t0, u0); u1 = fma(wz[z], t1, u1);                                                   \
+                }                                                                                                       \
+                double r = fma(wx2.y, u1, wx2.x * u0);                                                                  \
+                r += __shfl_xor_sync(0xffffffffu, r, 1);                                                                \
+                r += __shfl_xor_sync(0xffffffffu, r, 2);                                                                \
+                if (live && t == 0) atomicAdd(&psi[s.qidx[hr]], r);                                                     \
+            } else {                                                                                                    \
+                const double b0 = live ? w[DW + BR + t] : 0.0, b1 = live ? w[DW + BR + t + 4] : 0.0;  /* wy u_y */      \
+                const double2 wxu2 = *reinterpret_cast<const double2*>(w + BR + 2 * t);               /* wx u_x */      \
+                double wzu[BR];                                                                                         \
+                _Pragma("unroll") for (int z = 0; z < BR; z += 2) {                                                     \
+                    const double2 v = *reinterpret_cast<const double2*>(w + 2 * DW + BR + z);                           \
+                    wzu[z] = v.x; wzu[z + 1] = v.y;                                                                     \
+                }                                                                                                       \
+                double u0 = 0.0, u1 = 0.0, uz0 = 0.0, uz1 = 0.0, uy0 = 0.0, uy1 = 0.0;                                  \
+                _Pragma("unroll") for (int z = 0; z < BR; ++z) {                                                        \
+                    double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;                                                      \
+                    dmma884(t0, t1, a0, H[z][0]);                                                                       \
+                    dmma884(t0, t1, a1, H[z][1]);                                                                       \
+                    dmma884(v0, v1, b0, H[z][0]);                                                                       \
+                    dmma884(v0, v1, b1, H[z][1]);                                                                       \
+                    u0 = fma(wz[z], t0, u0); u1 = fma(wz[z], t1, u1);                                                   \
+                    uz0 = fma(wzu[z], t0, uz0); uz1 = fma(wzu[z], t1, uz1);                                             \
+                    uy0 = fma(wz[z], v0, uy0); uy1 = fma(wz[z], v1, uy1);                                               \
+                }                                                                                                       \
+                double r0 = fma(wx2.y, u1, wx2.x * u0);      /* psi                  */                                 \
+                double r1 = fma(wxu2.y, u1, wxu2.x * u0);    /* sum W u_x H          */                                 \
+                double r2 = fma(wx2.y, uy1, wx2.x * uy0);    /* sum W u_y H          */                                 \
+                double r3 = fma(wx2.y, uz1, wx2.x * uz0);    /* sum W u_z H          */                                 \
+                r0 += __shfl_xor_sync(0xffffffffu, r0, 1); r1 += __shfl_xor_sync(0xffffffffu, r1, 1);                   \
+                r2 += __shfl_xor_sync(0xffffffffu, r2, 1); r3 += __shfl_xor_sync(0xffffffffu, r3, 1);                   \
+                r0 += __shfl_xor_sync(0xffffffffu, r0, 2); r1 += __shfl_xor_sync(0xffffffffu, r1, 2);                   \
+                r2 += __shfl_xor_sync(0xffffffffu, r2, 2); r3 += __shfl_xor_sync(0xffffffffu, r3, 2);                   \
+                if (live) {                                                                                             \
+                    const int p = s.qidx[hr];                                                                           \
+                    /* E = -grad_a, dW/dx_a = +grad_fac u W; lane t issues quantity t */                                \
+                    if (t == 0) atomicAdd(&psi[p], r0);                                                                 \
+                    else if (t == 1) atomicAdd(&ex[p], -wc.grad_fac[0] * r1);                                           \
+                    else if (t == 2) atomicAdd(&ey[p], -wc.grad_fac[1] * r2);                                           \
+                    else atomicAdd(&ez[p], -wc.grad_fac[2] * r3);                                                       \
+                }                                                                                                       \
             }                                                                                                           \
         }                                                                                                               \
         __syncwarp();                                                                                                   \
