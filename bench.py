@@ -302,21 +302,34 @@ def run_ours(args, rank, world, local_rank):
     nm1, nfull = max(acc["n_matvec_bead"], 1), max(acc["n_eval_full"], 1)
     npairs = max(acc["n_fft_pairs"], 1)
 
-    def rf(ms_total, launches_, bytes_per_launch, bound="hbm"):
+    dfma_tf, dmma_tf = pce.measure_fp64_peaks()  # live, on this device (csrc/peaks.cu)
+    P3 = float(ctx.params.P) ** 3
+
+    def rf(ms_total, launches_, bytes_per_launch, fma_per_launch=None):
+        """HBM roofline of a pass; passes bound by fp64 arithmetic (fma_per_launch given: useful window updates, 2 flop each)
+        report "bound": "alu" against the measured fp64 mma peak and keep the HBM figures beside it."""
         if ms_total <= 0:
             return None
-        gbs = bytes_per_launch / (ms_total / launches_ * 1e-3) / 1e9
-        return {"bound": bound, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
-                "ms_per_launch": ms_total / launches_, "algorithmic_bytes": bytes_per_launch, "launches": launches_}
+        sec = ms_total / launches_ * 1e-3
+        gbs = bytes_per_launch / sec / 1e9
+        d = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+             "ms_per_launch": ms_total / launches_, "algorithmic_bytes": bytes_per_launch, "launches": launches_}
+        if fma_per_launch:
+            tf = 2.0 * fma_per_launch / sec / 1e12
+            d.update({"bound": "alu", "achieved": tf, "peak": dmma_tf, "unit": "TFLOP/s", "frac": tf / dmma_tf,
+                      "hbm_achieved_gbs": gbs, "hbm_frac": gbs / hbm_peak, "algorithmic_fma": fma_per_launch})
+        return d
     passes = {
-        "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3),
-        "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead),
+        "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3, w.N_bead * P3),
+        "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead, w.N_bead * P3),
         "real_bead_csr": rf(acc["bead_real"], nm1, 12 * info["nnz_near"] + 20 * w.N_bead),
         "scale": rf(acc["scale"], npairs, 32 * Nk),
         "fft_d2z(cuFFT)": rf(acc["fft"], npairs, 8 * Ng3 + 16 * Nk),
         "ifft_z2d(cuFFT)": rf(acc["ifft"], npairs, 8 * Ng3 + 16 * Nk),
-        "spread_full": rf(acc["spread"] - acc["bead_spread"], nfull, 32 * w.N + 8 * Ng3),
-        "gather_full_field": rf(acc["gather"] - acc["bead_gather"], nfull, 8 * Ng3 + 64 * w.N),
+        "spread_full": rf(acc["spread"] - acc["bead_spread"], nfull, 32 * w.N + 8 * Ng3, w.N * P3),
+        # per step: one potential-only gather at the beads (right-hand side) and one potential + field gather at all N
+        "gather_full": rf(acc["gather"] - acc["bead_gather"], nfull, 8 * Ng3 + (40 * w.N_bead + 64 * w.N) / 2,
+                          (w.N_bead + 4 * w.N) / 2 * P3),
     }
     own = {k: v for k, v in passes.items() if v and "cuFFT" not in k}
     dom = max(own, key=lambda k: own[k]["ms_per_launch"] * own[k]["launches"])
@@ -339,7 +352,8 @@ def run_ours(args, rank, world, local_rank):
         "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
                   "evals_full": acc["n_eval_full"], "rel_resid": sinfo["rel_resid"], "converged": sinfo["converged"]},
         "passes_ms_per_step": {k: acc[k] / args.steps for k in ("cells", "real", "spread", "fft", "scale", "ifft", "gather", "krylov", "other", "total")},
-        "roofline": roof, "roofline_passes": passes, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+        "roofline": roof, "roofline_passes": passes,
+        "fp64_peaks_tflops": {"dfma": dfma_tf, "mma_f64": dmma_tf, "how": "pce_measure_fp64_peaks: register-resident chains, this device, this run"}, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
     }
     if not args.no_cpu_baseline:
         import oracle as orc

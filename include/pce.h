@@ -76,7 +76,8 @@ typedef struct {
 typedef struct {
     int    iters;       /* Krylov iterations taken */
     int    matvecs;     /* applications of M inside pce_solve (bead-only + full) */
-    double rel_resid;   /* final |P(b - M q)| / (|P r.E0|^2 + |P psi0|^2)^(1/2) */
+    double rel_resid;   /* final |P(b - M q)| / (|P r.E0|^2 + |P psi0|^2)^(1/2), psi0 = potential of the uniform starting
+                           charges and the ions; a warm-started solve keeps the scale of the last cold solve if larger */
     int    converged;   /* 1 if rel_resid <= tol_solver */
 } pce_solve_info;
 
@@ -186,6 +187,10 @@ int pce_step_host(pce_ctx* ctx, const double* x, const double* y, const double* 
  * Heaviside term -- for n radii r[i] in [a/4, r_c); entries outside that range come back NaN (the device uses the
  * exact formula there).  All pointers host. */
 int pce_real_kernel_host(double a, double xi, double rc, double eps_f, int n, const double* r, double* R, double* dR);
+
+/* Measured fp64 roofs of the current device (register-resident chains, ~10 ms): tflops[0] = DFMA on the vector pipe,
+ * tflops[1] = mma.sync.m8n8k4.f64 on the tensor path.  Host pointer.  bench.py reports the spread / gather passes against them. */
+int pce_measure_fp64_peaks(double tflops[2]);
 
 int pce_set_timing(pce_ctx* ctx, int enabled);          /* per-pass CUDA events on/off (default off) */
 int pce_get_timings(const pce_ctx* ctx, pce_timings* t);

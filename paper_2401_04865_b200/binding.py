@@ -21,7 +21,7 @@ PCE_OK, PCE_EINVAL, PCE_ENOMEM, PCE_ECUDA, PCE_ECUFFT, PCE_ENOCONV, PCE_ESTATE =
 EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
-    "pce_get_info", "pce_launch_count", "pce_real_kernel_host",
+    "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks",
 )
 
 
@@ -87,6 +87,7 @@ def load():
     lib.pce_get_info.argtypes = [vp, C.POINTER(PceInfo)]
     lib.pce_launch_count.argtypes = [vp]
     lib.pce_launch_count.restype = C.c_longlong
+    lib.pce_measure_fp64_peaks.argtypes = [C.POINTER(C.c_double)]
     lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
@@ -106,6 +107,15 @@ def real_kernel_host(a, xi, rc, r, eps_f=1.0):
     if rc_ != PCE_OK:
         raise PceError(rc_, "pce_real_kernel_host: bad arguments")
     return R, dR
+
+
+def measure_fp64_peaks():
+    """(DFMA TFLOP/s, fp64 mma TFLOP/s) measured on the current CUDA device."""
+    out = (C.c_double * 2)()
+    rc_ = load().pce_measure_fp64_peaks(out)
+    if rc_ != PCE_OK:
+        raise PceError(rc_, "pce_measure_fp64_peaks failed (needs a CUDA device)")
+    return float(out[0]), float(out[1])
 
 
 def _d3(v):

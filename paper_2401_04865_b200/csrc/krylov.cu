@@ -271,7 +271,12 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
     PCE_CUDA(c, cudaMemcpyAsync(&ref2, sc + 0, sizeof(double), cudaMemcpyDeviceToHost, c->st));
     PCE_CUDA(c, cudaMemcpyAsync(&gg, sc + 1, sizeof(double), cudaMemcpyDeviceToHost, c->st));
     PCE_CUDA(c, cudaStreamSynchronize(c->st));
-    const double ref = (ref2 > 0.0) ? sqrt(ref2) : 1.0;
+    // Scale of the data: (|P r.E0|^2 + |P psi0|^2)^(1/2) with psi0 the potential of the uniform starting charges and the
+    // ions.  After a warm start psi0 is already nearly equipotential and that norm collapses, so the scale of the last cold
+    // solve of this system is kept and used whenever it is larger.
+    double ref = (ref2 > 0.0) ? sqrt(ref2) : 1.0;
+    if (!warm) c->cg_ref_cold = ref;
+    else if (c->cg_ref_cold > ref) ref = c->cg_ref_cold;
     const double tol = c->p.tol_solver;
     int it = 0;
     inf.rel_resid = sqrt(gg) / ref;

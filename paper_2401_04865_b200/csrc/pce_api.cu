@@ -85,6 +85,7 @@ static void free_system(pce_ctx* c)
     c->ev_psi = c->ev_ex = c->ev_ey = c->ev_ez = c->cg_scal = nullptr;
     c->hs_dev = nullptr; c->hs_dev_n = 0;
     c->have_system = false;
+    c->cg_ref_cold = 0.0;
 }
 
 extern "C" int pce_destroy(pce_ctx* c)

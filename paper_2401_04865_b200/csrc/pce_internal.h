@@ -118,6 +118,7 @@ struct pce_ctx {
     // Krylov vectors [Nbead]
     double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr, *cg_rhs = nullptr;
     double *ev_psi = nullptr, *ev_ex = nullptr, *ev_ey = nullptr, *ev_ez = nullptr;  // [N]
+    double cg_ref_cold = 0.0;   // residual scale of the last cold-start solve (see solve_cg)
     double* cg_scal = nullptr;  // [3*(max_iter+2) + 2 + 2*Nbody + 16]
     // block-Jacobi preconditioner (precond.cu)
     bool pc_on = false;

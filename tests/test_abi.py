@@ -19,7 +19,7 @@ def lib():
 def test_exports_match_header(lib):
     hdr = open(os.path.join(ROOT, "include", "pce.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(pce_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(pce_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(pce.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
