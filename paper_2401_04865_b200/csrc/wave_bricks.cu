@@ -274,7 +274,7 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 // Per brick and mesh plane z the spread is a dense contraction over the hits h of the brick:
 //     H_z[y][x] = sum_h (wy_h[y] q_h wz_h[z]) wx_h[x]  =  (A_z B)[y][x],  A_z = 8 x hits, B = hits x 8,
 // issued four hits at a time as one fp64 mma per plane: 8 DMUL + 8 DMMA per 4 hits instead of 16 DMUL + 64 DFMA.
-__global__ void __launch_bounds__(BWARPS * 32, 5)
+__global__ void __launch_bounds__(BWARPS * 32, 6)
 k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                 const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_, int* __restrict__ work_ctr)
@@ -344,7 +344,7 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
 // the 8 planes,  psi_h += sum_x wx_h[x] U[h][x]  (4-lane shuffle, one atomicAdd per hit and quantity).  With the field the
 // window-gradient sums (reading A3) reuse T_z with wz u_z and wx u_x, and need a second contraction with wy u_y.
 template <bool FIELD>
-__global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 5)
+__global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 6)
 k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                 const double* __restrict__ grid, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
