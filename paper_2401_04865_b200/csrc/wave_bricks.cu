@@ -158,7 +158,7 @@ __device__ __forceinline__ void brick_weights(const WaveConst& wc, const double*
 #pragma unroll
         for (int j = 0; j < BR; ++j) {
             const int r = r0 + j;
-            v[j] = (r >= 0 && r < P) ? pw : 0.0;
+            v[j] = ((unsigned)r < (unsigned)P) ? pw : 0.0;
             if (FIELD) vu[j] = v[j] * (u0 + (double)r);
             pw *= t;
             t *= g2;

@@ -246,3 +246,13 @@ def test_block_jacobi_preconditioner_same_solution_fewer_iterations(pce):
     assert rel(res[True][0], res[False][0]) < 1e-10
     assert np.abs(res[True][1] - res[False][1]).max() < 1e-10 * max(np.abs(res[False][1]).max(), 1.0)
     assert res[True][2] * 3 < res[False][2], (res[True][2], res[False][2])
+
+
+@pytest.mark.parametrize("Ng", [(33, 33, 33), (30, 36, 44), (24, 24, 24)])
+def test_operator_grids_off_the_brick_lattice(pce, Ng):
+    """Meshes that are not a multiple of the 8-point brick edge (partial bricks, generic window weights, scalar stores when
+    N_x is odd) or barely larger than the support (N_g - P < 8): same operator, same bars."""
+    w = wl.tiny_random(seed=13, n_body=2, n_ion=30, L=6.0, Ng=32, a=0.2, neutral=False)
+    w.Ng = np.array(Ng, dtype=np.int32)
+    e_psi, e_E, e_mv, _ = _check_operator(pce, w)
+    assert e_psi < TOL_FIELD and e_E < TOL_FIELD and e_mv < TOL_FIELD, (e_psi, e_E, e_mv)
