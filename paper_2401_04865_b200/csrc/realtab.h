@@ -58,15 +58,16 @@ RT_HD void rt_eval(const RealTable& T, double s, bool field, double& N, double& 
     const double t = (s - s0) * two_inv_w - 1.0;
     const int n = T.n_int;
     const double* c = T.tab + (key - T.key_lo);
-    double p = c[RT_DEG * n];
-#pragma unroll
-    for (int k = RT_DEG - 1; k >= 0; --k) p = p * t + c[k * n];
-    N = p;
+    // Estrin's scheme (degree 7): dependency depth 4 instead of 7 -- the hit loop of k_real_cells is latency-bound
+    static_assert(RT_DEG == 7, "rt_eval is written for degree 7");
+    const double t2 = t * t, t4 = t2 * t2;
+    {
+        const double p01 = c[1 * n] * t + c[0], p23 = c[3 * n] * t + c[2 * n], p45 = c[5 * n] * t + c[4 * n], p67 = c[7 * n] * t + c[6 * n];
+        N = (p67 * t2 + p45) * t4 + (p23 * t2 + p01);
+    }
     if (field) {
         const double* d = c + (RT_DEG + 1) * n;
-        double q = d[RT_DEG * n];
-#pragma unroll
-        for (int k = RT_DEG - 1; k >= 0; --k) q = q * t + d[k * n];
-        g = q;
+        const double p01 = d[1 * n] * t + d[0], p23 = d[3 * n] * t + d[2 * n], p45 = d[5 * n] * t + d[4 * n], p67 = d[7 * n] * t + d[6 * n];
+        g = (p67 * t2 + p45) * t4 + (p23 * t2 + p01);
     }
 }
