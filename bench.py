@@ -337,7 +337,7 @@ def run_ours(args, rank, world, local_rank):
     roof["kernel"] = dom
     roof["peak_source"] = peak_src
     roof["traffic"] = None  # dram bytes per launch from the committed ncu --set full capture (config 5 only)
-    tpath = os.path.join(ROOT, "profiles", "r1d_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "r1f_traffic.json")
     if args.config == 5 and os.path.exists(tpath):
         roof["traffic"] = json.load(open(tpath)).get(dom)
     line = {
