@@ -187,6 +187,14 @@ __global__ void k_gather3(int n, const int* __restrict__ perm, const double* __r
     xs[i] = x[j]; ys[i] = y[j]; zs[i] = z[j];
 }
 
+// out[cell] = number of 32-target chunks of the cell, out[ncell] = 0 (then scanned in place)
+__global__ void k_chunk_count(int ncell, const int* __restrict__ cell_start, int* __restrict__ out)
+{
+    const int cidx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cidx > ncell) return;
+    out[cidx] = (cidx < ncell) ? (cell_start[cidx + 1] - cell_start[cidx] + 31) / 32 : 0;
+}
+
 int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3])
 {
     bins_free(b);
@@ -211,6 +219,14 @@ int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3])
     return PCE_OK;
 }
 
+// real-space binnings also carry the chunk list of the direct pass
+int bins_alloc_chunks(pce_ctx* c, Bins& b)
+{
+    PCE_CUDA(c, cudaMalloc(&b.chunk_start, ((size_t)b.ncell + 1) * sizeof(int)));
+    c->bytes += (long long)(((size_t)b.ncell + 1) * 4);
+    return PCE_OK;
+}
+
 int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile)
 {
     int nc[3], range[3] = {1, 1, 1};
@@ -229,7 +245,7 @@ void bins_free(Bins& b)
 {
     cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp); cudaFree(b.inv);
     cudaFree(b.xs); cudaFree(b.ys); cudaFree(b.zs); cudaFree(b.qs);
-    cudaFree(b.ws0); cudaFree(b.wcf);
+    cudaFree(b.ws0); cudaFree(b.wcf); cudaFree(b.chunk_start);
     b = Bins();
 }
 
@@ -263,6 +279,12 @@ int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const doub
     }
     k_gather3<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, x, y, z, b.xs, b.ys, b.zs, b.inv);
     c->launches++;
+    if (b.chunk_start) {  // real-space binnings: work items of the direct pass = (cell, chunk of 32 targets)
+        k_chunk_count<<<cdiv(b.ncell + 1, 256), 256, 0, c->st>>>(b.ncell, b.cell_start, b.chunk_start);
+        c->launches++;
+        int rc = exclusive_scan(c, b.chunk_start, b.ncell + 1);
+        if (rc) return rc;
+    }
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
 }

@@ -268,6 +268,8 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     cell_layout(c->p, nc, range);
     if ((rc = bins_alloc(c, c->all, N, nc, range))) return rc;
     if ((rc = bins_alloc(c, c->bead, c->Nbead, nc, range))) return rc;
+    if ((rc = bins_alloc_chunks(c, c->all))) return rc;
+    if ((rc = bins_alloc_chunks(c, c->bead))) return rc;
     if ((rc = bins_alloc_tiles(c, c->wall, N, 8))) return rc;  // 8-point mesh bins = bricks of wave_bricks.cu
     if ((rc = bins_alloc_tiles(c, c->wbead, c->Nbead, 8))) return rc;
     if ((rc = wave_coef_alloc(c, c->wall))) return rc;

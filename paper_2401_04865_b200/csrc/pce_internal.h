@@ -33,6 +33,7 @@ struct Bins {
     int* cell_of = nullptr;     // [n]
     int* cell_start = nullptr;  // [ncell+1]
     int* cell_fill = nullptr;   // [ncell+1] scratch
+    int* chunk_start = nullptr; // [ncell+1] real-space binnings: first 32-target chunk of each cell (scan of ceil(n_cell/32))
     int* perm = nullptr;        // [n] sorted slot -> index in the subset
     int* perm_tmp = nullptr;    // [n]
     double *xs = nullptr, *ys = nullptr, *zs = nullptr;  // [n] sorted, wrapped
@@ -182,6 +183,7 @@ struct PassTimer {
 
 // cells.cu
 int bins_alloc(pce_ctx* c, Bins& b, int n, const int nc[3], const int range[3]);          // real-space cells
+int bins_alloc_chunks(pce_ctx* c, Bins& b);
 int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile);                                  // mesh tiles of `tile` grid points
 void bins_free(Bins& b);
 int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const double* z);

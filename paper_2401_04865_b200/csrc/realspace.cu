@@ -113,8 +113,8 @@ __device__ __forceinline__ void pair_eval(const RealConst& k, const RealTable& T
 }
 
 // ---------------------------------------------------------------- direct pass (step 1)
-// The paper runs one thread per particle over the neighbour cells.  Here one WARP owns a target cell: lane l owns
-// target l of a chunk of 32, the sources of each of the 27 neighbour cells (or periodic images, reading A10) are
+// The paper runs one thread per particle over the neighbour cells.  Here one WARP owns a chunk of up to 32 targets of one
+// cell (persistent warps, chunks handed out by a global counter): lane l owns target l, the sources of each of the 27 neighbour cells (or periodic images, reading A10) are
 // staged 64 at a time in the warp's shared memory by coalesced loads, every lane tests its target against the 64
 // staged sources (broadcast reads, 7 fp64 instructions per test) and records the hits in a 64-bit mask; the kernel
 // (two degree-7 polynomials from the table) is then evaluated hit by hit, so the expensive body runs max_lane(hits)
@@ -126,7 +126,8 @@ constexpr int RS_STAGE = 64;
 
 template <bool FIELD>
 __global__ void __launch_bounds__(RS_WARPS * 32)
-k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_start, const double* __restrict__ txs,
+k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_start, const int* __restrict__ t_chunk,
+             const double* __restrict__ txs,
              const double* __restrict__ tys, const double* __restrict__ tzs, const int* __restrict__ s_start,
              const double* __restrict__ sxs, const double* __restrict__ sys, const double* __restrict__ szs,
              const double* __restrict__ sqs, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
@@ -146,18 +147,24 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
     double2* szq = sh_zq[warp];
     const int ncell = g.nc[0] * g.nc[1] * g.nc[2];
     for (;;) {
-        int cell = 0;
-        if (lane == 0) cell = atomicAdd(work_ctr, 1);
-        cell = __shfl_sync(0xffffffffu, cell, 0);
-        if (cell >= ncell) return;
-        const int tb = t_start[cell], te = t_start[cell + 1];
-        if (te == tb) continue;
-        const int cx = cell % g.nc[0], cy = (cell / g.nc[0]) % g.nc[1], cz = cell / (g.nc[0] * g.nc[1]);
-        for (int t0 = tb; t0 < te; t0 += 32) {
-            const int i = t0 + lane;
-            const bool valid = i < te;
-            const double xi = valid ? txs[i] : 1e150, yi = valid ? tys[i] : 1e150, zi = valid ? tzs[i] : 1e150;
-            double a_psi = 0.0, a_x = 0.0, a_y = 0.0, a_z = 0.0;
+        // work item: one chunk of up to 32 targets of ONE cell (cells.cu scans ceil(n_cell/32) into t_chunk): a crowded cell
+        // is shared by many warps, a warp never straddles cells
+        int item = 0;
+        if (lane == 0) item = atomicAdd(work_ctr, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= t_chunk[ncell]) return;
+        int lo = 0, hi = ncell;  // largest cell with t_chunk[cell] <= item
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (t_chunk[mid] <= item) lo = mid; else hi = mid;
+        }
+        const int cell = lo;
+        const int i = t_start[cell] + 32 * (item - t_chunk[cell]) + lane;
+        const bool valid = i < t_start[cell + 1];
+        const double xi = valid ? txs[i] : 1e150, yi = valid ? tys[i] : 1e150, zi = valid ? tzs[i] : 1e150;
+        double a_psi = 0.0, a_x = 0.0, a_y = 0.0, a_z = 0.0;
+        {
+            const int cx = cell % g.nc[0], cy = (cell / g.nc[0]) % g.nc[1], cz = cell / (g.nc[0] * g.nc[1]);
             for (int oz = -g.range[2]; oz <= g.range[2]; ++oz) {
                 int nz = cz + oz;
                 const int wz = floor_div(nz, g.nc[2]);
@@ -216,10 +223,10 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
                     }
                 }
             }
-            if (valid) {
-                psi[i] = a_psi * k.inv_eps;
-                if (FIELD) { ex[i] = a_x * k.inv_eps; ey[i] = a_y * k.inv_eps; ez[i] = a_z * k.inv_eps; }
-            }
+        }
+        if (valid) {
+            psi[i] = a_psi * k.inv_eps;
+            if (FIELD) { ex[i] = a_x * k.inv_eps; ey[i] = a_y * k.inv_eps; ez[i] = a_z * k.inv_eps; }
         }
     }
 }
@@ -244,15 +251,15 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
     const size_t dyn = in_smem ? tab_bytes : 0;
     const int per_sm = in_smem ? (int)((200 * 1024) / (dyn + 8192 + 1024)) : 8;
     int blocks = c->num_sm * (per_sm < 1 ? 1 : per_sm > 8 ? 8 : per_sm);
-    const int need = cdiv(tb.ncell, RS_WARPS);
+    const int need = cdiv(cdiv(tb.n, 32) + tb.ncell, RS_WARPS);  // upper bound of the number of chunks
     if (blocks > need) blocks = need;
     if (field) {
         if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-        k_real_cells<true><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+        k_real_cells<true><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
                                                                    sb.xs, sb.ys, sb.zs, sb.qs, psi_s, ex_s, ey_s, ez_s, c->work_ctr + 1, in_smem);
     } else {
         if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-        k_real_cells<false><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
+        k_real_cells<false><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
                                                                     sb.xs, sb.ys, sb.zs, sb.qs, psi_s, nullptr, nullptr, nullptr, c->work_ctr + 1, in_smem);
     }
     c->launches++;
@@ -261,6 +268,7 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
 }
 
 // ---------------------------------------------------------------- cached near field (CSR)
+// ---- thread-per-row variants (few candidates per neighbour cell: a warp per row would idle most lanes)
 struct OpCount {
     int cnt = 0;
     __device__ __forceinline__ void operator()(int, double, double, double, double) { ++cnt; }
@@ -315,6 +323,84 @@ k_csr_fill(int n, CellGeom g, RealConst k, RealTable T, const int* __restrict__ 
     for_neighbors(g, cell_start, xs, ys, zs, i, k.rc2, op);
 }
 
+// ---- warp-per-row variants (crowded cells)
+// One warp per row (sorted bead i): the lanes test the candidates of the 27 neighbour cells 32 at a time; hits are counted
+// (k_csr_count) or ranked by ballot, evaluated one per lane and written in candidate order (k_csr_fill): every lane of the
+// warp evaluates a kernel, the row's entries are written with coalesced stores, and the order is fixed (deterministic SpMV).
+template <bool FILL>
+__global__ void __launch_bounds__(256)
+k_csr_rows(int n, CellGeom g, RealConst k, RealTable T, const int* __restrict__ cell_start, const double* __restrict__ xs,
+           const double* __restrict__ ys, const double* __restrict__ zs, int* __restrict__ row_ptr, int* __restrict__ col,
+           double* __restrict__ val, int tab_in_smem)
+{
+    extern __shared__ double sh_tab[];
+    if (FILL && tab_in_smem) {
+        const int nt = (RT_DEG + 1) * T.n_int;
+        for (int e = threadIdx.x; e < nt; e += blockDim.x) sh_tab[e] = T.tab[e];
+        __syncthreads();
+        T.tab = sh_tab;
+    }
+    const int lane = threadIdx.x & 31;
+    const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (i >= n) return;
+    const double xi = xs[i], yi = ys[i], zi = zs[i];
+    const int cx = min((int)(xi * g.inv_cell[0]), g.nc[0] - 1);
+    const int cy = min((int)(yi * g.inv_cell[1]), g.nc[1] - 1);
+    const int cz = min((int)(zi * g.inv_cell[2]), g.nc[2] - 1);
+    long long pos = 0;
+    int cnt = 1;  // the diagonal (self term, eq. 21) comes first
+    if (FILL) {
+        pos = row_ptr[i];
+        if (lane == 0) { col[pos] = i; val[pos] = k.R0 * k.inv_eps; }
+        ++pos;
+    }
+    for (int oz = -g.range[2]; oz <= g.range[2]; ++oz) {
+        int nz = cz + oz;
+        const int wz = floor_div(nz, g.nc[2]);
+        nz -= wz * g.nc[2];
+        const double sz = wz * g.L[2];
+        for (int oy = -g.range[1]; oy <= g.range[1]; ++oy) {
+            int ny = cy + oy;
+            const int wy = floor_div(ny, g.nc[1]);
+            ny -= wy * g.nc[1];
+            const double sy = wy * g.L[1];
+            for (int ox = -g.range[0]; ox <= g.range[0]; ++ox) {
+                int nx = cx + ox;
+                const int wx = floor_div(nx, g.nc[0]);
+                nx -= wx * g.nc[0];
+                const double sx = wx * g.L[0];
+                const int cell = (nz * g.nc[1] + ny) * g.nc[0] + nx;
+                const int jb = cell_start[cell], je = cell_start[cell + 1];
+                const bool home = (ox == 0 && oy == 0 && oz == 0);
+                for (int j0 = jb; j0 < je; j0 += 32) {
+                    const int j = j0 + lane;
+                    bool hit = false;
+                    double r2 = 0.0;
+                    if (j < je && !(home && j == i)) {
+                        const double dx = xi - (xs[j] + sx), dy = yi - (ys[j] + sy), dz = zi - (zs[j] + sz);
+                        r2 = dx * dx + dy * dy + dz * dz;
+                        hit = r2 < k.rc2;
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    if (FILL) {
+                        if (hit) {
+                            double R = k.R0, gk;
+                            if (r2 > 0.0) pair_eval(k, T, r2, false, R, gk);
+                            const long long w = pos + __popc(m & ((1u << lane) - 1u));
+                            col[w] = j;
+                            val[w] = R * k.inv_eps;
+                        }
+                        pos += __popc(m);
+                    } else {
+                        cnt += __popc(m);
+                    }
+                }
+            }
+        }
+    }
+    if (!FILL && lane == 0) row_ptr[i] = cnt;
+}
+
 int real_csr_build(pce_ctx* c, const Bins& b)
 {
     c->nnz = 0;
@@ -322,7 +408,14 @@ int real_csr_build(pce_ctx* c, const Bins& b)
     PassTimer t(c, PASS_REAL);
     const int n = b.n;
     PCE_CUDA(c, cudaMemsetAsync(c->csr_ptr + n, 0, sizeof(int), c->st));
-    k_csr_count<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk.rc2, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr);
+    // crowded cells (>= 32 particles per cell on average, e.g. one 2562-bead sphere inside a few r_c-sized cells) or few rows:
+    // one warp per row; otherwise one thread per row
+    const bool warp_rows = (double)n / b.ncell >= 32.0 || n < 32768;
+    if (warp_rows)
+        k_csr_rows<false><<<cdiv((long long)n * 32, 256), 256, 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs,
+                                                                            c->csr_ptr, nullptr, nullptr, 0);
+    else
+        k_csr_count<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk.rc2, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr);
     c->launches++;
     int rc = exclusive_scan(c, c->csr_ptr, n + 1);
     if (rc) return rc;
@@ -346,9 +439,15 @@ int real_csr_build(pce_ctx* c, const Bins& b)
     c->nnz = nnz;
     const size_t tab_bytes = (size_t)(RT_DEG + 1) * c->rt.n_int * sizeof(double);
     const int in_smem = tab_bytes <= 96 * 1024 ? 1 : 0;
-    if (in_smem && tab_bytes > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_csr_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_bytes));
-    k_csr_fill<<<cdiv(n, 128), 128, in_smem ? tab_bytes : 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr,
-                                                                      c->csr_col, c->csr_val, in_smem);
+    if (warp_rows) {
+        if (in_smem && tab_bytes > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_csr_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_bytes));
+        k_csr_rows<true><<<cdiv((long long)n * 32, 256), 256, in_smem ? tab_bytes : 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs,
+                                                                                                 b.ys, b.zs, c->csr_ptr, c->csr_col, c->csr_val, in_smem);
+    } else {
+        if (in_smem && tab_bytes > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_csr_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_bytes));
+        k_csr_fill<<<cdiv(n, 128), 128, in_smem ? tab_bytes : 0, c->st>>>(n, geom_of(b), c->rk, c->rt, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr,
+                                                                          c->csr_col, c->csr_val, in_smem);
+    }
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
