@@ -3,9 +3,9 @@
 //
 // The paper spreads with one block of P^3 threads per particle and global atomics
 // (PAPER.md:263).  Here the mesh is cut into 8^3 bricks and ONE WARP owns one brick: lane l
-// holds the 4x4 (x,y) patch at (x0,y0) = (4(l&1), 4((l>>1)&1)), z = l>>2 in 16 fp64
-// REGISTERS.  Warps never synchronise with each other (one __syncthreads after the table
-// load, none afterwards):
+// holds, for all 8 planes, the points (y = l/4, x = 2(l%4), 2(l%4)+1) in 16 fp64 REGISTERS
+// (the mma D / B fragment layout).  Warps never synchronise with each other (one
+// __syncthreads after the table load, none afterwards):
 //   1. particles are binned by 8-point mesh bin (counting sort, cells.cu; bins shifted by
 //      P/2 mod 8 so that the cells whose support meets a brick span ceil((P+7)/8) bins per
 //      dimension); the warp enumerates the contiguous runs of the sorted particle list in
@@ -20,12 +20,10 @@
 //      W(phi + 8m) = c0 e8^m exp(-aw (phi + 8m)^2), t(r) = e1 exp(-aw (2r + 1)); no exp here;
 //   4. accumulate on the fp64 tensor path (mma.sync m8n8k4.f64, measured 37.1 TFLOP/s against 33.3 for DFMA chains):
 //      per brick the spread is the contraction H_z[y][x] = sum_h (wy_h[y] q_h wz_h[z]) wx_h[x] over the hits h of
-//      the brick, the gather T_z[h][x] = sum_y wy_h[y] H~_z[y][x]; see the kernels.  The (x, y) patch per lane of
-//      the description above becomes the mma fragment layout: lane l holds (y = l/4, x = 2(l%4), 2(l%4)+1) of all 8 planes.
+//      the brick, the gather T_z[h][x] = sum_y wy_h[y] H~_z[y][x]; see the kernels.
 // Spread writes every mesh point exactly once (no atomics, no memset, deterministic).
-// Gather keeps the brick of H~ in registers, reduces the 32 lane partials of 8 hits (4 with
-// the field) at a time by a transposing butterfly and issues one global fp64 atomicAdd per
-// hit and quantity.  The window is the truncated Gaussian of eq. 25 on exactly the P^3
+// Gather keeps the brick of H~ in registers as the mma B operand, handles 8 hits per step and
+// issues one global fp64 atomicAdd per hit and quantity.  The window is the truncated Gaussian of eq. 25 on exactly the P^3
 // nearest mesh points (reading A5), identical in both passes, so the mesh operator stays
 // symmetric.  Grids with Ng % 8 != 0 or Ng - P < 8 take a generic weight routine (direct
 // exp, wrap-aware); everything else is shared.
