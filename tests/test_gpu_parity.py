@@ -256,3 +256,42 @@ def test_operator_grids_off_the_brick_lattice(pce, Ng):
     w.Ng = np.array(Ng, dtype=np.int32)
     e_psi, e_E, e_mv, _ = _check_operator(pce, w)
     assert e_psi < TOL_FIELD and e_E < TOL_FIELD and e_mv < TOL_FIELD, (e_psi, e_E, e_mv)
+
+
+def test_step_host_matches_the_device_calls(pce):
+    """pce_step_host (host buffers in, host buffers out: what bench.py's e2e times) = set_positions + solve + forces."""
+    import torch
+    w = wl.config2(d=2.5)
+    ctx, (x, y, z, Q, qi) = _ctx(pce, w)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    nb = w.N_body
+    host = {k: np.zeros(n) for k, n in (("q", w.N), ("Phi", nb), ("fx", w.N), ("fy", w.N), ("fz", w.N), ("F", 3 * nb), ("T", 3 * nb),
+                                         ("S", 3 * nb), ("U", 3))}
+    xs = [np.ascontiguousarray(w.x[:, k]) for k in range(3)]
+    si = ctx.step_host(xs[0], xs[1], xs[2], np.ascontiguousarray(w.Q_body), np.ascontiguousarray(w.q_ion), w.E0, host)
+    assert si["converged"] and si["iters"] == info["iters"]
+    assert rel(host["q"], q.cpu().numpy()) < 1e-13 and rel(host["Phi"], Phi.cpu().numpy()) < 1e-12
+    f = np.stack([host["fx"], host["fy"], host["fz"]], axis=1)
+    assert rel(f, out["f"].cpu().numpy()) < 1e-12
+    for key in ("F", "T", "S"):
+        ref = out[key].cpu().numpy()
+        assert np.abs(host[key].reshape(3, nb).T - ref).max() <= 1e-12 * max(np.abs(out["f"].cpu().numpy()).sum(0).max(), 1.0)
+    assert host["U"][1] == pytest.approx(float(out["W"]), rel=1e-12)
+    ctx.close()
+
+
+def test_operator_is_symmetric_on_the_mesh_path(pce):
+    """M is symmetric: x.(M y) = y.(M x) for the bead-only matvec (cached near field + spread/FFT/gather with one
+    window in both passes) and for the full evaluation -- a property that holds at any size (here config 4: 141 088 particles)."""
+    import torch
+    w = wl.config4()
+    ctx, _ = _ctx(pce, w)
+    gen = torch.Generator("cuda").manual_seed(3)
+    for n, apply in ((w.N_bead, ctx.matvec), (w.N, lambda v: ctx.evaluate(v, field=False))):
+        xv = torch.randn(n, dtype=torch.float64, device="cuda", generator=gen)
+        yv = torch.randn(n, dtype=torch.float64, device="cuda", generator=gen)
+        a, b = float(xv @ apply(yv)), float(yv @ apply(xv))
+        scale = float(torch.linalg.norm(xv) * torch.linalg.norm(apply(yv)))
+        assert abs(a - b) < 1e-11 * scale, (a, b, scale)
+    ctx.close()
