@@ -295,3 +295,49 @@ def test_operator_is_symmetric_on_the_mesh_path(pce):
         scale = float(torch.linalg.norm(xv) * torch.linalg.norm(apply(yv)))
         assert abs(a - b) < 1e-11 * scale, (a, b, scale)
     ctx.close()
+
+
+def test_large_body_falls_back_to_scaled_identity_preconditioner(pce):
+    """Bodies above 4096 beads get no dense preconditioner block (scaled identity instead): mixed with a 642-bead body that has
+    one, the preconditioned solve must still reach the solution of the plain CG solve (unique: M is SPD)."""
+    from workloads import geometry as geo
+    from workloads.configs import _mk
+    small, big = geo.icosphere(3), geo.icosphere(5)
+    a = geo.bead_radius(big)
+    beads = np.concatenate([small + np.array([5.0, 5.0, 2.8]), big + np.array([5.0, 5.0, 7.3])])
+    w = _mk("mixed_body_sizes", beads, [0, len(small), len(small) + len(big)], [0.3, -0.3], np.zeros((0, 3)), np.zeros(0),
+            [0.2, 0.0, 1.0], 10.0, 64, a)
+    res = {}
+    for pc in (True, False):
+        ctx = pce.context_for(w, tol=1e-8, precond=pc)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        assert ctx.info()["n_precond_blocks"] == (1 if pc else 0)
+        q, Phi, info = ctx.solve(Q, qi, w.E0)
+        assert info["converged"], info
+        res[pc] = (q.cpu().numpy(), info["iters"])
+        ctx.close()
+    assert rel(res[True][0], res[False][0]) < 1e-9
+    assert res[True][1] < res[False][1]
+
+
+def test_set_system_twice_on_one_context(pce):
+    """A context can be re-used for another system of the same box: nothing of the first system (cell lists, near field,
+    preconditioner, residual scale) leaks into the second."""
+    w1 = wl.tiny_random(seed=21, n_body=3, n_ion=20, L=6.0, Ng=32, a=0.2)
+    w2 = wl.tiny_random(seed=22, n_body=2, n_ion=35, L=6.0, Ng=32, a=0.2)
+    ctx = pce.context_for(w1)
+    outs = []
+    for w in (w1, w2, w1):
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        q, Phi, info = ctx.solve(Q, qi, w.E0)
+        outs.append(q.cpu().numpy())
+    ctx.close()
+    ctx2 = pce.context_for(w2)
+    x, y, z, Q, qi = pce.upload(w2)
+    ctx2.set_system(w2.body_offset, x, y, z)
+    q2, _, _ = ctx2.solve(Q, qi, w2.E0)
+    ctx2.close()
+    assert rel(outs[1], q2.cpu().numpy()) < 1e-13
+    assert rel(outs[2], outs[0]) < 1e-13
