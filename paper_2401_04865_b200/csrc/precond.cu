@@ -246,25 +246,41 @@ k_pc_apply(const PcRows* __restrict__ rows, const float* __restrict__ Bm, const 
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool vec = (R.n % 4 == 0);
-#pragma unroll 1
-    for (int k = 0; k < PC_ROWS / 8; ++k) {
-        const int row = R.row0 + warp + 8 * k;
-        if (row >= R.n) break;
-        const float* Br = Bm + R.boff + (long long)row * R.n;
-        double s0 = 0.0, s1 = 0.0;
-        if (vec) {
-            for (int j = 4 * lane; j < R.n; j += 128) {
-                const float4 b = *reinterpret_cast<const float4*>(Br + j);
-                s0 = fma((double)b.x, sr[j], s0); s1 = fma((double)b.y, sr[j + 1], s1);
-                s0 = fma((double)b.z, sr[j + 2], s0); s1 = fma((double)b.w, sr[j + 3], s1);
-            }
-        } else {
-            for (int j = lane; j < R.n; j += 32) s0 = fma((double)Br[j], sr[j], s0);
-        }
-        double s = s0 + s1;
+    // the warp's 4 rows are swept together: one read of the residual from shared memory serves 4 rows, and 4 independent
+    // 16-byte loads are in flight per lane
+    constexpr int NR = PC_ROWS / 8;
+    const float* Br[NR];
+    bool live[NR];
+    double acc[NR];
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-        if (lane == 0) z[R.j0 + row] = s;
+    for (int k = 0; k < NR; ++k) {
+        const int row = R.row0 + warp + 8 * k;
+        live[k] = row < R.n;
+        Br[k] = Bm + R.boff + (long long)(live[k] ? row : 0) * R.n;
+        acc[k] = 0.0;
+    }
+    if (vec) {
+        for (int j = 4 * lane; j < R.n; j += 128) {
+            const double2 r01 = *reinterpret_cast<const double2*>(sr + j), r23 = *reinterpret_cast<const double2*>(sr + j + 2);
+#pragma unroll
+            for (int k = 0; k < NR; ++k) {
+                const float4 b = *reinterpret_cast<const float4*>(Br[k] + j);
+                acc[k] = fma((double)b.x, r01.x, fma((double)b.y, r01.y, fma((double)b.z, r23.x, fma((double)b.w, r23.y, acc[k]))));
+            }
+        }
+    } else {
+        for (int j = lane; j < R.n; j += 32) {
+            const double rj = sr[j];
+#pragma unroll
+            for (int k = 0; k < NR; ++k) acc[k] = fma((double)Br[k][j], rj, acc[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NR; ++k) {
+        double sum = acc[k];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+        if (lane == 0 && live[k]) z[R.j0 + R.row0 + warp + 8 * k] = sum;
     }
 }
 
