@@ -56,6 +56,7 @@ typedef enum {
 
 /* pce_params.flags */
 #define PCE_FLAG_NO_PRECOND 1  /* plain (unpreconditioned) conjugate gradients in pce_solve */
+#define PCE_FLAG_CUFFT_3D   2  /* 3-D cuFFT plans + separate scaling pass instead of 2-D cuFFT per plane + fused z pass */
 
 /* Parameters of the spectral Ewald sum and of the solver.
  * eta is NOT a free input: eta = h^2 xi^2 P / pi (eq. 31,

@@ -94,7 +94,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     cudaStreamSynchronize(c->st);
     free_system(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -153,8 +153,18 @@ static int create_impl(pce_ctx* c)
     c->have_plans = true;
     cufftSetAutoAllocation(c->planF, 0);
     cufftSetAutoAllocation(c->planB, 0);
-    if (cufftMakePlan3d(c->planF, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_D2Z, &wsF) != CUFFT_SUCCESS ||
-        cufftMakePlan3d(c->planB, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_Z2D, &wsB) != CUFFT_SUCCESS) {
+    c->use_zfft = zfft_supported(p) && !(p.flags & PCE_FLAG_CUFFT_3D);
+    if (c->use_zfft) {  // (x, y) transforms per mesh plane by cuFFT, the z axis fused with the scaling (zfft.cu)
+        int dims[2] = {p.Ng[1], p.Ng[0]};
+        if (cufftMakePlanMany(c->planF, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, p.Ng[2], &wsF) != CUFFT_SUCCESS ||
+            cufftMakePlanMany(c->planB, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_Z2D, p.Ng[2], &wsB) != CUFFT_SUCCESS) {
+            c->err = "cuFFT cannot plan this grid";
+            return PCE_ECUFFT;
+        }
+        int rcz = zfft_init(c);
+        if (rcz) return rcz;
+    } else if (cufftMakePlan3d(c->planF, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_D2Z, &wsF) != CUFFT_SUCCESS ||
+               cufftMakePlan3d(c->planB, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_Z2D, &wsB) != CUFFT_SUCCESS) {
         c->err = "cuFFT cannot plan this grid";
         return PCE_ECUFFT;
     }

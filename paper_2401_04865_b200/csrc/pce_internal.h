@@ -106,6 +106,9 @@ struct pce_ctx {
     cufftHandle planF = 0, planB = 0;
     void* fft_work = nullptr;
     bool have_plans = false;
+    bool use_zfft = false;     // 2-D cuFFT per plane + fused z FFT / Green's function / inverse z FFT (zfft.cu)
+    double2* ztw = nullptr;    // twiddles exp(-2 pi i m / N_z)
+    double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
     int* work_ctr = nullptr;
@@ -202,6 +205,11 @@ int realtab_upload(pce_ctx* c);
 
 // wave.cu
 int wave_fft_scale_ifft(pce_ctx* c);
+
+// zfft.cu
+bool zfft_supported(const pce_params& p);
+int zfft_init(pce_ctx* c);
+int zfft_scale(pce_ctx* c);
 
 // wave_bricks.cu
 int wave_bricks_init(pce_ctx* c);

@@ -56,7 +56,11 @@ int wave_fft_scale_ifft(pce_ctx* c)
         PassTimer t(c, PASS_FFT);
         if (cufftExecD2Z(c->planF, c->grid, c->gridk) != CUFFT_SUCCESS) { c->err = "cufftExecD2Z failed"; return PCE_ECUFFT; }
     }
-    {
+    if (c->use_zfft) {
+        PassTimer t(c, PASS_SCALE);  // z FFT + Green's function + inverse z FFT in one pass over the half spectrum
+        int rc = zfft_scale(c);
+        if (rc) return rc;
+    } else {
         PassTimer t(c, PASS_SCALE);
         const size_t total = (size_t)c->wk.Nxh * (c->wk.Ng[1] / 2 + 1) * (c->wk.Ng[2] / 2 + 1);
         const int blocks = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);

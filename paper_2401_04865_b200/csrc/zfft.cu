@@ -1,0 +1,234 @@
+// zfft.cu -- steps 3-5 of the spectral Ewald algorithm with the z axis fused:
+//   cuFFT 2-D D2Z per mesh plane (x, y)  ->  k_zfft_scale: FFT along z, multiply by the Green's function of eq. 26
+//   (PAPER.md:219), inverse FFT along z, all in shared memory  ->  cuFFT 2-D Z2D per plane.
+// The separate passes (cuFFT z pass, k_scale, cuFFT z pass) move the 1.08 GB half spectrum through HBM three times
+// (6 x 1.08 GB at 512^3); fused, it is read once and written once.  cuFFT stays the only library call and does the
+// (x, y) transforms.  Available for power-of-two N_z in 16..1024; other meshes use the 3-D cuFFT plans + k_scale (wave.cu).
+//
+// Layout: gk[z][y][kx] complex128.  A CTA owns a tile of KP = 4 consecutive kx of one row y (64 contiguous bytes per z) and then
+// the mirror row N_y - y, for which the Green's function values are the same (computed once per CTA into shared memory, the
+// Gaussian factor from per-axis host tables).  Thread (j, p): pencil p = kx0 + p, butterfly index j.  Shared tile [z][KP]: the
+// pencils of a z are consecutive, so every warp access is conflict-free.
+// Stockham autosort, radix 8 (the rest radix 4 or 2), in place with a barrier between the loads and the stores of a stage;
+// the first forward stage reads global memory, the last inverse stage writes it.  Twiddles exp(-2 pi i m / N) come from a
+// host-computed table.  The z transform pair needs no particular sign convention: the Green's function is even in k_z.
+#include "pce_internal.h"
+
+#include <cmath>
+
+namespace {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+// multiply by s i  (s = -1: forward, e^{-2 pi i ...})
+template <int S> __device__ __forceinline__ double2 cmuli(double2 a) { return (S < 0) ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x); }
+
+// X[k] = sum_n x[n] W^{nk}, W = exp(S 2 pi i / R), natural order in and out
+template <int S> __device__ __forceinline__ void dft2(double2* v)
+{
+    const double2 a = v[0], b = v[1];
+    v[0] = cadd(a, b); v[1] = csub(a, b);
+}
+template <int S> __device__ __forceinline__ void dft4(double2* c)
+{
+    const double2 t0 = cadd(c[0], c[2]), t1 = csub(c[0], c[2]), t2 = cadd(c[1], c[3]), t3 = cmuli<S>(csub(c[1], c[3]));
+    c[0] = cadd(t0, t2); c[2] = csub(t0, t2); c[1] = cadd(t1, t3); c[3] = csub(t1, t3);
+}
+template <int S> __device__ __forceinline__ void dft8(double2* x)
+{
+    const double h = 0.70710678118654752440;
+    double2 a[4], b[4];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) { a[n] = cadd(x[n], x[n + 4]); b[n] = csub(x[n], x[n + 4]); }
+    // b[n] *= W^n, W = exp(S i pi / 4): W^1 = (1 + S i)/sqrt2, W^2 = S i, W^3 = (-1 + S i)/sqrt2
+    b[1] = make_double2(h * (b[1].x - S * b[1].y), h * (b[1].y + S * b[1].x));
+    b[2] = cmuli<S>(b[2]);
+    b[3] = make_double2(h * (-b[3].x - S * b[3].y), h * (-b[3].y + S * b[3].x));
+    dft4<S>(a);
+    dft4<S>(b);
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { x[2 * m] = a[m]; x[2 * m + 1] = b[m]; }
+}
+template <int R, int S> __device__ __forceinline__ void dftR(double2* v)
+{
+    if (R == 8) dft8<S>(v);
+    else if (R == 4) dft4<S>(v);
+    else dft2<S>(v);
+}
+
+// One Stockham stage of radix R on the thread's 8 elements (8/R butterflies).  in/out: element i of the pencil at
+// base[i * stride].  Loads (with the optional per-element scale g, radix 8 only), barrier if in place, stores.
+template <int N, int R, int S, bool SYNC>
+__device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok, double2* out, size_t ostr, bool out_ok, int Ns, int j,
+                                      const double2* __restrict__ tw, const double* g)
+{
+    constexpr int NB = 8 / R;          // butterflies per thread
+    constexpr int NT = N / 8;          // threads per pencil
+    double2 v[8];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int b = j + q * NT;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double2 e = in_ok ? in[(size_t)(b + r * (N / R)) * istr] : make_double2(0.0, 0.0);
+            if (g) { e.x *= g[r]; e.y *= g[r]; }
+            v[q * R + r] = e;
+        }
+    }
+    if (SYNC) __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int b = j + q * NT;
+        const int k = b & (Ns - 1);
+        const int tstep = k * (N / (Ns * R));
+#pragma unroll
+        for (int r = 1; r < R; ++r) {
+            double2 w = tw[r * tstep];
+            if (S > 0) w.y = -w.y;
+            v[q * R + r] = cmul(v[q * R + r], w);
+        }
+        dftR<R, S>(v + q * R);
+        const int d = (b - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (out_ok) out[(size_t)(d + r * Ns) * ostr] = v[q * R + r];
+    }
+}
+
+template <int N> struct Radices {
+    static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;  // N = 8^m * rest
+    static constexpr int n8 = (N == 16 || N == 32 || N == 64) ? (N == 64 ? 2 : 1) : (N == 128 || N == 256 || N == 512) ? (N == 512 ? 3 : 2) : 3;
+};
+
+// forward (S = -1): stages 8 (global -> smem), 8.., rest (-> smem);  inverse (S = +1): 8 (smem, scaled -> smem), 8.., rest (-> global)
+// KP pencils per CTA, N/8 threads per pencil.  zexp = [ex | ey | ez]: exp(-gexp_d k_d^2) per axis (host tables).
+constexpr int KP = 4;
+template <int N>
+__global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
+k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp)
+{
+    extern __shared__ __align__(16) unsigned char zsm[];
+    double2* tile = reinterpret_cast<double2*>(zsm);       // [N][KP]
+    double2* tw = tile + (size_t)N * KP;                    // [N]
+    double* gs = reinterpret_cast<double*>(tw + N);         // [N][KP] Green's function of the CTA's pencils
+    constexpr int REST = Radices<N>::rest, N8 = Radices<N>::n8;
+    const int tid = threadIdx.x, p = tid % KP, j = tid / KP;
+    for (int i = tid; i < N; i += N / 8 * KP) tw[i] = tw_g[i];
+    const int nxh = wc.Nxh, ny = wc.Ng[1];
+    const int kxi = blockIdx.x * KP + p, iy = blockIdx.y;  // iy in [0, ny/2]
+    const bool col_ok = kxi < nxh;
+    const size_t zstr = (size_t)ny * nxh;
+    // Green's function (eq. 26, with all constants folded in) at this thread's 8 k_z: element i = j + r N/8 of the spectrum;
+    // the same values serve the row iy and its mirror N_y - iy
+    {
+        const double kx = wc.kfac[0] * kxi, ky = wc.kfac[1] * iy;
+        const double kx2 = kx * kx, ky2 = ky * ky;
+        const double exy = col_ok ? wc.scale_norm * zexp[kxi] * zexp[nxh + iy] : 0.0;
+        const double* ez = zexp + nxh + ny / 2 + 1;
+#pragma unroll 2
+        for (int r = 0; r < 8; ++r) {
+            const int i = j + r * (N / 8);
+            const int iz = i <= N / 2 ? i : N - i;
+            const double kz = wc.kfac[2] * (double)iz;
+            const double k2 = kx2 + ky2 + kz * kz;
+            double f = 0.0;  // k = 0 removed
+            if (k2 > 0.0 && col_ok) {
+                const double ka = sqrt(k2) * wc.a;
+                const double j0 = (ka < 1e-4) ? 1.0 - ka * ka * (1.0 / 6.0) : sin(ka) / ka;
+                f = exy * ez[iz] * j0 * j0 / k2;
+            }
+            gs[i * KP + p] = f;
+        }
+    }
+    const int my = (iy == 0 || 2 * iy == ny) ? -1 : ny - iy;  // mirror row: same |k_y|
+    for (int pass = 0; pass < 2; ++pass) {
+        const int y = pass == 0 ? iy : my;
+        if (y < 0) break;
+        double2* col = gk + (size_t)y * nxh + (col_ok ? kxi : 0);
+        double2* sp = tile + p;
+        __syncthreads();  // twiddles and Green's function stored / previous pass done with the tile
+        double g[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) g[r] = gs[(j + r * (N / 8)) * KP + p];
+        // ---- forward
+        stage<N, 8, -1, false>(col, zstr, col_ok, sp, KP, true, 1, j, tw, nullptr);
+        __syncthreads();
+        int Ns = 8;
+        if (N8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (N8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (REST != 8) { stage<N, REST, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); }
+        // ---- scale + inverse
+        if (REST != 8 || N8 > 1) {
+            stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, 1, j, tw, g);
+            __syncthreads();
+            Ns = 8;
+            if (N8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+            if (REST != 8) {
+                if (N8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+                stage<N, REST, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
+            } else {
+                stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
+            }
+        }
+    }
+}
+
+template <int N> int launch(pce_ctx* c)
+{
+    const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set && smem > 48 * 1024) {
+        PCE_CUDA(c, cudaFuncSetAttribute(k_zfft_scale<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    const dim3 grid(cdiv(c->wk.Nxh, KP), c->wk.Ng[1] / 2 + 1);
+    k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+}  // namespace
+
+bool zfft_supported(const pce_params& p)
+{
+    const int n = p.Ng[2];
+    return (n == 16 || n == 32 || n == 64 || n == 128 || n == 256 || n == 512 || n == 1024) && p.Ng[1] % 2 == 0;
+}
+
+// twiddle table exp(-2 pi i m / N_z) (host, long double) and the two batched 2-D cuFFT plans
+int zfft_init(pce_ctx* c)
+{
+    const int n = c->p.Ng[2];
+    std::vector<double2> tw(n);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int m = 0; m < n; ++m) tw[m] = make_double2((double)cosl(-2.0L * pi * m / n), (double)sinl(-2.0L * pi * m / n));
+    PCE_CUDA(c, cudaMalloc(&c->ztw, n * sizeof(double2)));
+    PCE_CUDA(c, cudaMemcpy(c->ztw, tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice));
+    // per-axis factors exp(-(1 - eta_d) k_d^2 / 4 xi^2) of eq. 26: [kx = 0..Nx/2 | ky = 0..Ny/2 | kz = 0..Nz/2]
+    const int cnt[3] = {c->wk.Nxh, c->p.Ng[1] / 2 + 1, n / 2 + 1};
+    std::vector<double> ze;
+    for (int d = 0; d < 3; ++d)
+        for (int i = 0; i < cnt[d]; ++i) {
+            const double k = c->wk.kfac[d] * i;
+            ze.push_back(std::exp(-c->wk.gexp[d] * k * k));
+        }
+    PCE_CUDA(c, cudaMalloc(&c->zexp, ze.size() * sizeof(double)));
+    PCE_CUDA(c, cudaMemcpy(c->zexp, ze.data(), ze.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return PCE_OK;
+}
+
+int zfft_scale(pce_ctx* c)
+{
+    switch (c->p.Ng[2]) {
+        case 16: return launch<16>(c);
+        case 32: return launch<32>(c);
+        case 64: return launch<64>(c);
+        case 128: return launch<128>(c);
+        case 256: return launch<256>(c);
+        case 512: return launch<512>(c);
+        case 1024: return launch<1024>(c);
+        default: c->err = "zfft_scale: unsupported N_z"; return PCE_EINVAL;
+    }
+}
