@@ -82,11 +82,29 @@ __device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok
         const int b = j + q * NT;
         const int k = b & (Ns - 1);
         const int tstep = k * (N / (Ns * R));
-#pragma unroll
-        for (int r = 1; r < R; ++r) {
-            double2 w = tw[r * tstep];
-            if (S > 0) w.y = -w.y;
-            v[q * R + r] = cmul(v[q * R + r], w);
+        if (tstep != 0) {
+            // twiddles w^r, w = exp(S 2 pi i k / (Ns R)): w, w^2, w^4 from the table (three loads instead of seven: threads of
+            // a warp read different k, i.e. conflicting banks), the rest by products
+            double2 w1 = tw[tstep];
+            if (S > 0) w1.y = -w1.y;
+            if (R == 2) {
+                v[q * R + 1] = cmul(v[q * R + 1], w1);
+            } else {
+                double2 w2 = tw[2 * tstep];
+                if (S > 0) w2.y = -w2.y;
+                const double2 w3 = cmul(w1, w2);
+                v[q * R + 1] = cmul(v[q * R + 1], w1);
+                v[q * R + 2] = cmul(v[q * R + 2], w2);
+                v[q * R + 3] = cmul(v[q * R + 3], w3);
+                if (R == 8) {
+                    double2 w4 = tw[4 * tstep];
+                    if (S > 0) w4.y = -w4.y;
+                    v[q * R + 4] = cmul(v[q * R + 4], w4);
+                    v[q * R + 5] = cmul(v[q * R + 5], cmul(w4, w1));
+                    v[q * R + 6] = cmul(v[q * R + 6], cmul(w4, w2));
+                    v[q * R + 7] = cmul(v[q * R + 7], cmul(w4, w3));
+                }
+            }
         }
         dftR<R, S>(v + q * R);
         const int d = (b - k) * R + k;
@@ -119,26 +137,25 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
     const int kxi = blockIdx.x * KP + p, iy = blockIdx.y;  // iy in [0, ny/2]
     const bool col_ok = kxi < nxh;
     const size_t zstr = (size_t)ny * nxh;
-    // Green's function (eq. 26, with all constants folded in) at this thread's 8 k_z: element i = j + r N/8 of the spectrum;
-    // the same values serve the row iy and its mirror N_y - iy
+    // Green's function (eq. 26, with all constants folded in) of the CTA's pencils into shared memory.  It is even in k_z and
+    // in k_y: N/2 + 1 evaluations per pencil serve both halves of the spectrum and both rows (iy and its mirror N_y - iy).
     {
-        const double kx = wc.kfac[0] * kxi, ky = wc.kfac[1] * iy;
-        const double kx2 = kx * kx, ky2 = ky * ky;
-        const double exy = col_ok ? wc.scale_norm * zexp[kxi] * zexp[nxh + iy] : 0.0;
+        const double ky = wc.kfac[1] * iy;
         const double* ez = zexp + nxh + ny / 2 + 1;
-#pragma unroll 2
-        for (int r = 0; r < 8; ++r) {
-            const int i = j + r * (N / 8);
-            const int iz = i <= N / 2 ? i : N - i;
-            const double kz = wc.kfac[2] * (double)iz;
-            const double k2 = kx2 + ky2 + kz * kz;
-            double f = 0.0;  // k = 0 removed
-            if (k2 > 0.0 && col_ok) {
-                const double ka = sqrt(k2) * wc.a;
-                const double j0 = (ka < 1e-4) ? 1.0 - ka * ka * (1.0 / 6.0) : sin(ka) / ka;
-                f = exy * ez[iz] * j0 * j0 / k2;
+        for (int e = tid; e < (N / 2 + 1) * KP; e += N / 8 * KP) {
+            const int iz = e / KP, pp = e % KP, kxe = blockIdx.x * KP + pp;
+            double f = 0.0;  // k = 0 removed; pencils beyond N_x/2 unused
+            if (kxe < nxh) {
+                const double kx = wc.kfac[0] * kxe, kz = wc.kfac[2] * (double)iz;
+                const double k2 = kx * kx + ky * ky + kz * kz;
+                if (k2 > 0.0) {
+                    const double ka = sqrt(k2) * wc.a;
+                    const double j0 = (ka < 1e-4) ? 1.0 - ka * ka * (1.0 / 6.0) : sin(ka) / ka;
+                    f = wc.scale_norm * zexp[kxe] * zexp[nxh + iy] * ez[iz] * j0 * j0 / k2;
+                }
             }
-            gs[i * KP + p] = f;
+            gs[iz * KP + pp] = f;
+            if (iz > 0 && iz < N / 2) gs[(N - iz) * KP + pp] = f;
         }
     }
     const int my = (iy == 0 || 2 * iy == ny) ? -1 : ny - iy;  // mirror row: same |k_y|
