@@ -94,7 +94,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     cudaStreamSynchronize(c->st);
     free_system(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;

@@ -109,6 +109,8 @@ struct pce_ctx {
     bool use_zfft = false;     // 2-D cuFFT per plane + fused z FFT / Green's function / inverse z FFT (zfft.cu)
     double2* ztw = nullptr;    // twiddles exp(-2 pi i m / N_z)
     double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function
+    double* zshape = nullptr;  // piecewise-polynomial table of the shape factor j0(ka)^2 / k^2 as a function of k^2
+    int zshape_key_lo = 0, zshape_n = 0;
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
     int* work_ctr = nullptr;
@@ -202,6 +204,8 @@ int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s);
 // realtab.cu
 void realtab_build_host(double a, double xi, double rc, std::vector<double>& tab, RealTable& T);
 int realtab_upload(pce_ctx* c);
+void chebtab_build(double s_lo, double s_hi, long double (*f)(long double, const void*), const void* ctx, std::vector<double>& tab,
+                   int& key_lo, int& n_int);
 
 // wave.cu
 int wave_fft_scale_ifft(pce_ctx* c);

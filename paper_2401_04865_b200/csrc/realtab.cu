@@ -103,6 +103,33 @@ void realtab_build_host(double a, double xi, double rc, std::vector<double>& tab
     T.tab = tab.data();
 }
 
+// Generic table of one smooth function f(s), s in [s_lo', s_hi], with the interval scheme of realtab.h, interval-major:
+// tab[interval][RT_DEG + 1] monomial coefficients in t.  Used for the shape factor of the Green's function (zfft.cu).
+void chebtab_build(double s_lo, double s_hi, long double (*f)(long double, const void*), const void* ctx, std::vector<double>& tab,
+                   int& key_lo, int& n_int)
+{
+    int e = 0;
+    std::frexp(s_lo, &e);
+    const double lo = std::ldexp(1.0, e - 1);  // largest power of two <= s_lo
+    key_lo = key_of(lo);
+    n_int = key_of(s_hi * (1.0 + 1e-12)) - key_lo + 1;
+    if (n_int < 1) n_int = 1;
+    constexpr int n = RT_DEG + 1;
+    tab.assign((size_t)n_int * n, 0.0);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int i = 0; i < n_int; ++i) {
+        const int key = key_lo + i;
+        const long double s0 = rt_from_hi(key << (20 - RT_BITS));
+        const long double w = ldexpl(1.0L, (key >> RT_BITS) - 1023 - RT_BITS);
+        long double fv[n];
+        for (int j = 0; j < n; ++j) {
+            const long double t = cosl(pi * (j + 0.5L) / n);
+            fv[j] = f(s0 + 0.5L * (t + 1.0L) * w, ctx);
+        }
+        cheb_fit(fv, &tab[(size_t)i * n]);
+    }
+}
+
 int realtab_upload(pce_ctx* c)
 {
     std::vector<double> tab;

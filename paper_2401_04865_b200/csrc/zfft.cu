@@ -114,6 +114,21 @@ __device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok
     }
 }
 
+// j0(ka)^2 / k^2 at s = k^2 > 0: degree-7 polynomial of the interval of s (intervals follow the floating-point format of s,
+// 16 per octave, as in realtab.h; host table in long double, zfft_init)
+__device__ __forceinline__ double shape_eval(const double* __restrict__ tab, int key_lo, double s)
+{
+    const int key = __double2hiint(s) >> (20 - RT_BITS);
+    const double s0 = __hiloint2double(key << (20 - RT_BITS), 0);
+    const double two_inv_w = __hiloint2double((2047 + RT_BITS - (key >> RT_BITS)) << 20, 0);
+    const double t = (s - s0) * two_inv_w - 1.0;
+    const double* c = tab + (size_t)(key - key_lo) * (RT_DEG + 1);
+    const double2 c01 = __ldg(reinterpret_cast<const double2*>(c)), c23 = __ldg(reinterpret_cast<const double2*>(c + 2));
+    const double2 c45 = __ldg(reinterpret_cast<const double2*>(c + 4)), c67 = __ldg(reinterpret_cast<const double2*>(c + 6));
+    const double t2 = t * t, t4 = t2 * t2;
+    return ((c67.y * t + c67.x) * t2 + (c45.y * t + c45.x)) * t4 + ((c23.y * t + c23.x) * t2 + (c01.y * t + c01.x));
+}
+
 template <int N> struct Radices {
     static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;  // N = 8^m * rest
     static constexpr int n8 = (N == 16 || N == 32 || N == 64) ? (N == 64 ? 2 : 1) : (N == 128 || N == 256 || N == 512) ? (N == 512 ? 3 : 2) : 3;
@@ -124,7 +139,8 @@ template <int N> struct Radices {
 constexpr int KP = 4;
 template <int N>
 __global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
-k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp)
+k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
+             const double* __restrict__ shape, int shape_key_lo)
 {
     extern __shared__ __align__(16) unsigned char zsm[];
     double2* tile = reinterpret_cast<double2*>(zsm);       // [N][KP]
@@ -148,11 +164,8 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
             if (kxe < nxh) {
                 const double kx = wc.kfac[0] * kxe, kz = wc.kfac[2] * (double)iz;
                 const double k2 = kx * kx + ky * ky + kz * kz;
-                if (k2 > 0.0) {
-                    const double ka = sqrt(k2) * wc.a;
-                    const double j0 = (ka < 1e-4) ? 1.0 - ka * ka * (1.0 / 6.0) : sin(ka) / ka;
-                    f = wc.scale_norm * zexp[kxe] * zexp[nxh + iy] * ez[iz] * j0 * j0 / k2;
-                }
+                if (k2 > 0.0)  // shape factor j0(ka)^2 / k^2 from its table in k^2 (no sqrt, sin or division here)
+                    f = wc.scale_norm * zexp[kxe] * zexp[nxh + iy] * ez[iz] * shape_eval(shape, shape_key_lo, k2);
             }
             gs[iz * KP + pp] = f;
             if (iz > 0 && iz < N / 2) gs[(N - iz) * KP + pp] = f;
@@ -200,7 +213,8 @@ template <int N> int launch(pce_ctx* c)
         attr_set = true;
     }
     const dim3 grid(cdiv(c->wk.Nxh, KP), c->wk.Ng[1] / 2 + 1);
-    k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp);
+    k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp, c->zshape,
+                                                        c->zshape_key_lo);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -233,6 +247,22 @@ int zfft_init(pce_ctx* c)
         }
     PCE_CUDA(c, cudaMalloc(&c->zexp, ze.size() * sizeof(double)));
     PCE_CUDA(c, cudaMemcpy(c->zexp, ze.data(), ze.size() * sizeof(double), cudaMemcpyHostToDevice));
+    // shape factor j0(ka)^2 / k^2 (eq. 9 / eq. 26) as a function of s = k^2 between the smallest and the largest mesh wavenumber
+    double smin = 1e300, smax = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        const double k1 = c->wk.kfac[d], kn = c->wk.kfac[d] * (c->p.Ng[d] / 2);
+        smin = std::fmin(smin, k1 * k1);
+        smax += kn * kn;
+    }
+    const long double a = c->p.a;
+    std::vector<double> st;
+    chebtab_build(smin, smax, [](long double s, const void* ctx) -> long double {
+        const long double x = *static_cast<const long double*>(ctx) * sqrtl(s);
+        const long double j0 = (x < 1e-6L) ? 1.0L - x * x / 6.0L : sinl(x) / x;
+        return j0 * j0 / s;
+    }, &a, st, c->zshape_key_lo, c->zshape_n);
+    PCE_CUDA(c, cudaMalloc(&c->zshape, st.size() * sizeof(double)));
+    PCE_CUDA(c, cudaMemcpy(c->zshape, st.data(), st.size() * sizeof(double), cudaMemcpyHostToDevice));
     return PCE_OK;
 }
 
