@@ -348,6 +348,8 @@ def run_ours(args, rank, world, local_rank):
                    "P": int(ctx.params.P), "xi": ctx.params.xi, "rc": ctx.params.rc, "ewald_tol": args.tol,
                    "solver_tol": args.tol_solver, "cells": info["ncell"], "nnz_near": info["nnz_near"],
                    "l2": "flushed between timed steps" if l2_flush is not None else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
+                   "fft": "cuFFT 2-D D2Z/Z2D per mesh plane; the 'scale' pass is the fused z FFT + Green's function + inverse z FFT kernel"
+                          if int(w.Ng[2]) in (16, 32, 64, 128, 256, 512, 1024) else "cuFFT 3-D D2Z/Z2D + separate scale pass",
                    "multi_gpu": "replicas only"},
         "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
                   "evals_full": acc["n_eval_full"], "rel_resid": sinfo["rel_resid"], "converged": sinfo["converged"]},
