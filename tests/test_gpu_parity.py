@@ -343,7 +343,7 @@ def test_set_system_twice_on_one_context(pce):
     assert rel(outs[2], outs[0]) < 1e-13
 
 
-@pytest.mark.parametrize("Ng", [(32, 32, 32), (64, 32, 128), (40, 48, 16)])
+@pytest.mark.parametrize("Ng", [(32, 32, 32), (64, 32, 128), (40, 48, 16), (32, 32, 256), (24, 32, 512)])
 def test_fused_z_pass_matches_the_3d_cufft_path(pce, Ng):
     """2-D cuFFT per plane + fused (z FFT, Green's function of eq. 26, inverse z FFT) kernel against the 3-D cuFFT plans +
     separate scaling pass: the same operator to rounding."""
