@@ -193,6 +193,10 @@ int pce_real_kernel_host(double a, double xi, double rc, double eps_f, int n, co
  * tflops[1] = mma.sync.m8n8k4.f64 on the tensor path.  Host pointer.  bench.py reports the spread / gather passes against them. */
 int pce_measure_fp64_peaks(double tflops[2]);
 
+/* Test hook: overwrite the shared memory of every SM with NaN bit patterns (on `stream`, a cudaStream_t), so that a kernel
+ * reading shared memory it never wrote poisons its result visibly.  No effect on any context. */
+int pce_debug_poison_shared_memory(void* stream);
+
 int pce_set_timing(pce_ctx* ctx, int enabled);          /* per-pass CUDA events on/off (default off) */
 int pce_get_timings(const pce_ctx* ctx, pce_timings* t);
 int pce_get_info(const pce_ctx* ctx, pce_info* info);

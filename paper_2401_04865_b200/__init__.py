@@ -3,6 +3,6 @@ shell-regularized Coulomb operator, on-device induced-charge solve, forces and
 torques.  The product is the CUDA library behind include/pce.h; this package is
 its build script and a thin ctypes binding (argument marshalling only)."""
 from .binding import (  # noqa: F401
-    Context, PceError, PceParams, context_for, suggest_params, real_kernel_host, measure_fp64_peaks, upload, load, lib_path, EXPORTS,
+    Context, PceError, PceParams, context_for, suggest_params, real_kernel_host, measure_fp64_peaks, poison_shared_memory, upload, load, lib_path, EXPORTS,
 )
 from .build import build  # noqa: F401

@@ -21,7 +21,7 @@ PCE_OK, PCE_EINVAL, PCE_ENOMEM, PCE_ECUDA, PCE_ECUFFT, PCE_ENOCONV, PCE_ESTATE =
 EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
-    "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks",
+    "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks", "pce_debug_poison_shared_memory",
 )
 
 
@@ -88,6 +88,7 @@ def load():
     lib.pce_launch_count.argtypes = [vp]
     lib.pce_launch_count.restype = C.c_longlong
     lib.pce_measure_fp64_peaks.argtypes = [C.POINTER(C.c_double)]
+    lib.pce_debug_poison_shared_memory.argtypes = [vp]
     lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
@@ -116,6 +117,14 @@ def measure_fp64_peaks():
     if rc_ != PCE_OK:
         raise PceError(rc_, "pce_measure_fp64_peaks failed (needs a CUDA device)")
     return float(out[0]), float(out[1])
+
+
+def poison_shared_memory():
+    """Test hook: fill every SM's shared memory with NaN patterns on the current torch stream."""
+    import torch
+    rc_ = load().pce_debug_poison_shared_memory(C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc_ != PCE_OK:
+        raise PceError(rc_, "pce_debug_poison_shared_memory failed")
 
 
 def _d3(v):

@@ -5,6 +5,8 @@
 // (PAPER.md:137-163).  All reductions have a fixed order (deterministic).
 #include "pce_internal.h"
 
+#include <cstdlib>
+
 constexpr int BT = 256;  // threads of the per-body / reduction blocks
 
 __device__ __forceinline__ double block_sum(double v, double* sh)
@@ -19,24 +21,6 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
     const int nw = (blockDim.x + 31) >> 5;
     for (int i = 0; i < nw; ++i) s += sh[i];
     return s;
-}
-
-// out[0] = sum(in[0..n))   (single block, fixed order)
-__global__ void __launch_bounds__(1024) k_sum(const double* __restrict__ in, long long n, double* __restrict__ out)
-{
-    __shared__ double sh[32];
-    double v = 0.0;
-    for (long long i = threadIdx.x; i < n; i += blockDim.x) v += in[i];
-    const double s = block_sum(v, sh);
-    if (threadIdx.x == 0) out[0] = s;
-}
-
-static int sum_to(pce_ctx* c, const double* in, long long n, double* out)
-{
-    k_sum<<<1, 1024, 0, c->st>>>(in, n, out);
-    c->launches++;
-    PCE_CUDA(c, cudaGetLastError());
-    return PCE_OK;
 }
 
 __device__ __forceinline__ double min_img(double d, double L) { return d - L * floor(d / L + 0.5); }
@@ -76,10 +60,50 @@ int bodies_setup(pce_ctx* c)
     return PCE_OK;
 }
 
-// ---------------------------------------------------------------- CG pieces
-// initial charges: beads Q_i/N_i (or the caller's guess re-centred so that sum_j q_ij = Q_i), ions fixed
+// ---------------------------------------------------------------- Krylov solve, whole iteration on the device
+// Conjugate gradients for eq. 13 with the ions eliminated (one-bead bodies of fixed charge):
+//     P M_bb P q = P b  on  Sigma q = Q,   P = I - Sigma^T (Sigma Sigma^T)^-1 Sigma  (subtract the per-body mean),
+// preconditioned by the rigid-body blocks of precond.cu; with project = 0 the same loop solves the plain SPD system
+// M_bb q = b (columns of the grand capacitance tensor, eq. 15).  All step lengths, the stopping test and the iteration
+// count live in CgState on the device; every sum is a per-block partial followed by a fixed-order sum in the block that
+// arrives last (deterministic, no extra launch).  One iteration is 5 own kernels + the operator and is replayed as a CUDA
+// graph; once converged every kernel of a replay returns at once.  The host never synchronises inside the loop: it
+// watches CgHostStatus (pinned, mapped) and keeps `depth` iterations in flight.
+
+// true (for the whole block) in the block that arrives last; the counter is left at 0 for the next use
+__device__ __forceinline__ bool last_block_done(unsigned* counter, unsigned nblocks)
+{
+    __shared__ bool last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(counter, 1u);
+        last = (t == nblocks - 1);
+        if (last) *counter = 0u;
+    }
+    __syncthreads();
+    if (last) __threadfence();
+    return last;
+}
+
+__device__ __forceinline__ double fixed_sum(const double* part, int n, double* sh)
+{
+    double v = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) v += part[i];
+    return block_sum(v, sh);
+}
+
+__device__ __forceinline__ void report(const CgState* st, CgHostStatus* hs)
+{
+    hs->gg = st->gg; hs->ref = st->ref;
+    __threadfence_system();
+    hs->it = st->it; hs->done = st->done;
+    __threadfence_system();
+}
+
+// initial charges: beads Q_i/N_i (or the caller's guess re-centred so that sum_j q_ij = Q_i)
 __global__ void __launch_bounds__(BT)
-k_init_q(const int* __restrict__ off, const double* __restrict__ Qb, int warm, double* __restrict__ q)
+k_init_q(const int* __restrict__ off, const double* __restrict__ Qb, int warm, const double* __restrict__ q_in, double* __restrict__ q)
 {
     __shared__ double sh[32];
     const int b = blockIdx.x;
@@ -89,10 +113,10 @@ k_init_q(const int* __restrict__ off, const double* __restrict__ Qb, int warm, d
     double mean = 0.0;
     if (warm) {
         double s = 0.0;
-        for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += q[j];
+        for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += q_in[j];
         mean = block_sum(s, sh) / (j1 - j0);
     }
-    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) q[j] = warm ? (q[j] - mean + uni) : uni;
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) q[j] = warm ? (q_in[j] - mean + uni) : uni;
 }
 
 __global__ void k_copy(int n, const double* __restrict__ in, double* __restrict__ out)
@@ -101,44 +125,158 @@ __global__ void k_copy(int n, const double* __restrict__ in, double* __restrict_
     if (i < n) out[i] = in[i];
 }
 
-// g = P(r.E0 - psi0), p = g; per-body partials of |g|^2 and of the reference norm
+// g = P(r.E0 - psi0) (one CTA per body); the last block sets up the solver state: |g|^2, the residual scale
+//   ref^2 = |P r.E0|^2 + |P psi0|^2 + 1e-4 |psi0|^2
+// (psi0 = potential of the starting charges and the ions; the unprojected term keeps the scale meaningful when psi0 is
+// already nearly equipotential, e.g. an isolated charged body without field), warm starts keep the scale of the last cold solve.
 __global__ void __launch_bounds__(BT)
-k_resid_init(const int* __restrict__ off, const double* __restrict__ rx, const double* __restrict__ ry, const double* __restrict__ rz,
-             double e0x, double e0y, double e0z, const double* __restrict__ psi0, double* __restrict__ rhs, double* __restrict__ g,
-             double* __restrict__ p, double* __restrict__ part_gg, double* __restrict__ part_ref)
+k_resid_init(int nb, const int* __restrict__ off, const double* __restrict__ rx, const double* __restrict__ ry, const double* __restrict__ rz,
+             double e0x, double e0y, double e0z, const double* __restrict__ psi0, double* __restrict__ g, double* __restrict__ part,
+             CgState* __restrict__ st, CgHostStatus* __restrict__ hs, int warm, int have_pc, double tol, int maxit)
 {
     __shared__ double sh[32];
     const int b = blockIdx.x;
     const int j0 = off[b], j1 = off[b + 1];
-    if (j1 <= j0) { if (threadIdx.x == 0) { part_gg[b] = 0; part_ref[b] = 0; } return; }
     double s = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += psi0[j];
-    const double mean = block_sum(s, sh) / (j1 - j0);
-    double gg = 0.0, rf = 0.0;
+    const double mean = (j1 > j0) ? block_sum(s, sh) / (j1 - j0) : 0.0;
+    double gg = 0.0, rf = 0.0, pp = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         const double re = rx[j] * e0x + ry[j] * e0y + rz[j] * e0z;  // sum_j r_ij = 0, so P(r.E0) = r.E0
-        const double pc = psi0[j] - mean;
+        const double p0 = psi0[j], pc = p0 - mean;
         const double v = re - pc;
-        rhs[j] = re; g[j] = v; p[j] = v;
-        gg += v * v; rf += re * re + pc * pc;
+        g[j] = v;
+        gg += v * v; rf += re * re + pc * pc; pp += p0 * p0;
     }
     gg = block_sum(gg, sh);
     rf = block_sum(rf, sh);
-    if (threadIdx.x == 0) { part_gg[b] = gg; part_ref[b] = rf; }
+    pp = block_sum(pp, sh);
+    if (threadIdx.x == 0) { part[b] = gg; part[nb + b] = rf; part[2 * nb + b] = pp; }
+    if (!last_block_done(&st->cnt[0], gridDim.x)) return;
+    const double tgg = fixed_sum(part, nb, sh), trf = fixed_sum(part + nb, nb, sh), tpp = fixed_sum(part + 2 * nb, nb, sh);
+    if (threadIdx.x == 0) {
+        const double r2 = trf + 1e-4 * tpp;
+        double ref = (r2 > 0.0) ? sqrt(r2) : 1.0;
+        if (!warm) st->ref_cold = ref;
+        else if (st->ref_cold > ref) ref = st->ref_cold;
+        st->ref = ref; st->gg = tgg; st->tol = tol; st->maxit = maxit; st->it = 0; st->project = 1; st->psum = 0.0; st->pap = 0.0;
+        st->rz[0] = tgg; st->rz[1] = tgg;
+        st->done = (!(sqrt(tgg) > tol * ref) || maxit <= 0) ? 1 : 0;   // NaN counts as done (reported as not converged)
+        if (!have_pc || st->done) report(st, hs);
+    }
 }
 
-// ap = P t ; partial of p.ap
+// plain system M q = b from q = 0: g = b; ref = |b|
 __global__ void __launch_bounds__(BT)
-k_proj_dot(const int* __restrict__ off, const double* __restrict__ t, const double* __restrict__ p, double* __restrict__ ap,
-           double* __restrict__ part)
+k_resid_init_plain(int n, const double* __restrict__ b, double* __restrict__ g, double* __restrict__ q, double* __restrict__ psi,
+                   double* __restrict__ part, CgState* __restrict__ st, CgHostStatus* __restrict__ hs, int have_pc, double tol, int maxit)
 {
+    __shared__ double sh[32];
+    double gg = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const double v = b[i];
+        g[i] = v; q[i] = 0.0; psi[i] = 0.0;
+        gg += v * v;
+    }
+    gg = block_sum(gg, sh);
+    if (threadIdx.x == 0) part[blockIdx.x] = gg;
+    if (!last_block_done(&st->cnt[0], gridDim.x)) return;
+    const double tgg = fixed_sum(part, gridDim.x, sh);
+    if (threadIdx.x == 0) {
+        st->ref = (tgg > 0.0) ? sqrt(tgg) : 1.0;
+        st->gg = tgg; st->tol = tol; st->maxit = maxit; st->it = 0; st->project = 0; st->psum = 0.0; st->pap = 0.0;
+        st->rz[0] = tgg; st->rz[1] = tgg;
+        st->done = (!(sqrt(tgg) > tol * st->ref) || maxit <= 0) ? 1 : 0;
+        if (!have_pc || st->done) report(st, hs);
+    }
+}
+
+// z = preconditioned residual, per body (one CTA):  project: z_raw - <z_raw>_body;  plain: z_raw + u (u.g)/(1.u)  (A^-1 from its
+// projected part B, precond.cu);  without a preconditioner z = g.  Partial of g.z; the last block stores g.z at rz[it & 1].
+__global__ void __launch_bounds__(BT)
+k_pc_dot(int nb, const int* __restrict__ off, double* __restrict__ zraw, const double* __restrict__ g, const double* __restrict__ u,
+         const double* __restrict__ inv_s, double* __restrict__ zmean, double* __restrict__ part, CgState* __restrict__ st,
+         CgHostStatus* __restrict__ hs, int report_init)
+{
+    if (st->done) return;
     __shared__ double sh[32];
     const int b = blockIdx.x;
     const int j0 = off[b], j1 = off[b + 1];
-    if (j1 <= j0) { if (threadIdx.x == 0) part[b] = 0; return; }
+    const int project = st->project;
+    double s = 0.0, d = 0.0, ug = 0.0;
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        const double z = zraw[j], gj = g[j];
+        s += z; d += gj * z; ug += u[j] * gj;
+    }
+    s = block_sum(s, sh);
+    d = block_sum(d, sh);
+    if (project) {
+        if (threadIdx.x == 0) zmean[b] = (j1 > j0) ? s / (j1 - j0) : 0.0;  // g has zero mean per body: g.z = g.z_raw
+    } else {
+        ug = block_sum(ug, sh);
+        const double cfac = ug * inv_s[b];  // 0 for bodies without a dense block
+        for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) zraw[j] += cfac * u[j];
+        d += cfac * ug;
+        if (threadIdx.x == 0) zmean[b] = 0.0;
+    }
+    if (threadIdx.x == 0) part[b] = d;
+    if (!last_block_done(&st->cnt[1], gridDim.x)) return;
+    const double t = fixed_sum(part, nb, sh);
+    if (threadIdx.x == 0) {
+        st->rz[st->it & 1] = t;
+        if (report_init) report(st, hs);
+    }
+}
+
+// p = z + beta p, beta = rz_new / rz_old (p = z in the first iteration), written in caller order and scattered into the two
+// sorted orders the operator reads (real-space cells, mesh bins); partial of sum(p) for the k = 0 constant
+__global__ void __launch_bounds__(256)
+k_pupdate(int n, const double* __restrict__ g, const double* __restrict__ zraw, const double* __restrict__ zmean,
+          const int* __restrict__ body_of, const int* __restrict__ inv_r, const int* __restrict__ inv_w, double* __restrict__ p,
+          double* __restrict__ qs_r, double* __restrict__ qs_w, double* __restrict__ part, CgState* __restrict__ st)
+{
+    if (st->done) return;
+    __shared__ double sh[32];
+    const int it = st->it;
+    double beta = 0.0;
+    if (it > 0) {
+        const double o = st->rz[(it + 1) & 1];
+        beta = (o != 0.0) ? st->rz[it & 1] / o : 0.0;
+    }
+    double ps = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const double z = zraw ? zraw[i] - zmean[body_of[i]] : g[i];
+        const double v = (it > 0) ? z + beta * p[i] : z;
+        p[i] = v;
+        qs_r[inv_r[i]] = v;
+        qs_w[inv_w[i]] = v;
+        ps += v;
+    }
+    ps = block_sum(ps, sh);
+    if (threadIdx.x == 0) part[blockIdx.x] = ps;
+    if (!last_block_done(&st->cnt[2], gridDim.x)) return;
+    const double t = fixed_sum(part, gridDim.x, sh);
+    if (threadIdx.x == 0) st->psum = t;
+}
+
+// t = M p assembled from the sorted real- and wave-space parts (step "a8", reading A1), ap = P t (or t), partial of p.ap
+__global__ void __launch_bounds__(BT)
+k_proj_dot(int nb, const int* __restrict__ off, const int* __restrict__ inv_r, const int* __restrict__ inv_w, const double* __restrict__ re,
+           const double* __restrict__ wa, double kconst, const double* __restrict__ p, double* __restrict__ t, double* __restrict__ ap,
+           double* __restrict__ part, CgState* __restrict__ st)
+{
+    if (st->done) return;
+    __shared__ double sh[32];
+    const int b = blockIdx.x;
+    const int j0 = off[b], j1 = off[b + 1];
+    const double shift = kconst * st->psum;
     double s = 0.0;
-    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += t[j];
-    const double mean = block_sum(s, sh) / (j1 - j0);
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        const double v = re[inv_r[j]] + wa[inv_w[j]] - shift;
+        t[j] = v;
+        s += v;
+    }
+    const double mean = (st->project && j1 > j0) ? block_sum(s, sh) / (j1 - j0) : 0.0;
     double d = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         const double v = t[j] - mean;
@@ -147,19 +285,24 @@ k_proj_dot(const int* __restrict__ off, const double* __restrict__ t, const doub
     }
     d = block_sum(d, sh);
     if (threadIdx.x == 0) part[b] = d;
+    if (!last_block_done(&st->cnt[3], gridDim.x)) return;
+    const double tt = fixed_sum(part, nb, sh);
+    if (threadIdx.x == 0) st->pap = tt;
 }
 
-// alpha = (g.z)/pAp ; q += alpha p ; g -= alpha ap ; psi += alpha t ; partial of |g|^2
+// alpha = (g.z)/(p.Ap); q += alpha p; psi += alpha t; g -= alpha ap; the last block: |g|^2, iteration count, stopping test
 __global__ void __launch_bounds__(BT)
-k_cg_update(const int* __restrict__ off, const double* __restrict__ sc_gg, const double* __restrict__ sc_pap,
-            const double* __restrict__ p, const double* __restrict__ ap, const double* __restrict__ t, double* __restrict__ q,
-            double* __restrict__ g, double* __restrict__ psi, double* __restrict__ part)
+k_cg_update(int nb, const int* __restrict__ off, const double* __restrict__ p, const double* __restrict__ ap, const double* __restrict__ t,
+            double* __restrict__ q, double* __restrict__ g, double* __restrict__ psi, double* __restrict__ part, CgState* __restrict__ st,
+            CgHostStatus* __restrict__ hs, int have_pc)
 {
+    if (st->done) return;
     __shared__ double sh[32];
     const int b = blockIdx.x;
     const int j0 = off[b], j1 = off[b + 1];
-    const double pap = sc_pap[0];
-    const double alpha = (pap != 0.0) ? sc_gg[0] / pap : 0.0;
+    const int it = st->it;
+    const double pap = st->pap;
+    const double alpha = (pap != 0.0) ? st->rz[it & 1] / pap : 0.0;
     double gg = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         q[j] += alpha * p[j];
@@ -170,38 +313,15 @@ k_cg_update(const int* __restrict__ off, const double* __restrict__ sc_gg, const
     }
     gg = block_sum(gg, sh);
     if (threadIdx.x == 0) part[b] = gg;
-}
-
-// beta = rz_new/rz_old (0 on the first call) ; p = z + beta p with z = g (no preconditioner) or
-// z = z_raw - <z_raw>_body (block-Jacobi, precond.cu)
-__global__ void k_cg_pupdate(int n, const double* __restrict__ sc_old, const double* __restrict__ sc_new, const double* __restrict__ g,
-                             const double* __restrict__ zraw, const double* __restrict__ zmean, const int* __restrict__ body_of,
-                             double* __restrict__ p)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    double beta = 0.0;
-    if (sc_old) {
-        const double o = sc_old[0];
-        beta = (o != 0.0) ? sc_new[0] / o : 0.0;
+    if (!last_block_done(&st->cnt[4], gridDim.x)) return;
+    const double tg = fixed_sum(part, nb, sh);
+    if (threadIdx.x == 0) {
+        st->gg = tg;
+        st->it = it + 1;
+        if (!have_pc) st->rz[(it + 1) & 1] = tg;
+        if (!(sqrt(tg) > st->tol * st->ref) || it + 1 >= st->maxit) st->done = 1;
+        report(st, hs);
     }
-    const double z = zraw ? zraw[i] - zmean[body_of[i]] : g[i];
-    p[i] = sc_old ? z + beta * p[i] : z;
-}
-
-// per body: mean of z_raw and the partial of g.z (g has zero mean per body, so g.z = g.z_raw)
-__global__ void __launch_bounds__(BT)
-k_pc_dot(const int* __restrict__ off, const double* __restrict__ zraw, const double* __restrict__ g, double* __restrict__ zmean,
-         double* __restrict__ part)
-{
-    __shared__ double sh[32];
-    const int b = blockIdx.x;
-    const int j0 = off[b], j1 = off[b + 1];
-    double s = 0.0, d = 0.0;
-    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) { const double z = zraw[j]; s += z; d += g[j] * z; }
-    s = block_sum(s, sh);
-    d = block_sum(d, sh);
-    if (threadIdx.x == 0) { zmean[b] = (j1 > j0) ? s / (j1 - j0) : 0.0; part[b] = d; }
 }
 
 // Phi_i = <psi_ij - r_ij.E0>_i = <psi_ij>_i
@@ -217,16 +337,165 @@ k_body_mean(const int* __restrict__ off, const double* __restrict__ v, double* _
     if (threadIdx.x == 0) out[b] = (j1 > j0) ? s / (j1 - j0) : 0.0;
 }
 
+static int pupdate_blocks(const pce_ctx* c) { int b = cdiv(c->Nbead, 256 * 4); return b < 1 ? 1 : (b > 1024 ? 1024 : b); }
+
+static int krylov_alloc(pce_ctx* c)
+{
+    if (c->cg_state) return PCE_OK;
+    PCE_CUDA(c, cudaMalloc(&c->cg_state, sizeof(CgState)));
+    PCE_CUDA(c, cudaMemset(c->cg_state, 0, sizeof(CgState)));
+    PCE_CUDA(c, cudaHostAlloc(&c->cg_host, sizeof(CgHostStatus), cudaHostAllocMapped));
+    PCE_CUDA(c, cudaHostGetDevicePointer(&c->cg_host_dev, c->cg_host, 0));
+    c->cg_host->it = 0; c->cg_host->done = 0; c->cg_host->gg = 0.0; c->cg_host->ref = 1.0;
+    return PCE_OK;
+}
+
+void krylov_invalidate_graph(pce_ctx* c)
+{
+    if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+}
+
+void krylov_free(pce_ctx* c)
+{
+    krylov_invalidate_graph(c);
+    cudaFree(c->cg_state);
+    if (c->cg_host) cudaFreeHost(c->cg_host);
+    c->cg_state = nullptr; c->cg_host = nullptr; c->cg_host_dev = nullptr; c->cg_graph_failed = false;
+}
+
+// the preconditioned residual and g.z for the current g (also used once before the loop)
+static int enqueue_precond(pce_ctx* c, int report_init)
+{
+    int rc = precond_apply(c, c->cg_g, c->cg_z);
+    if (rc) return rc;
+    k_pc_dot<<<c->Nbody, BT, 0, c->st>>>(c->Nbody, c->body_off, c->cg_z, c->cg_g, c->pc_u, c->pc_invs, c->pc_mean, c->cg_part, c->cg_state,
+                                        c->cg_host_dev, report_init);
+    c->launches++;
+    return PCE_OK;
+}
+
+// one iteration: search direction, operator, step.  Every kernel returns at once when the state says "done".
+static int enqueue_iteration(pce_ctx* c)
+{
+    const int nb = c->Nbody, n = c->Nbead;
+    const bool pc = c->pc_on;
+    int rc;
+    c->skip_flag = &c->cg_state->done;
+    {
+        PassTimer t(c, PASS_KRYLOV);
+        k_pupdate<<<pupdate_blocks(c), 256, 0, c->st>>>(n, c->cg_g, pc ? c->cg_z : nullptr, c->pc_mean, c->body_of, c->bead.inv, c->wbead.inv,
+                                                        c->cg_p, c->bead.qs, c->wbead.qs, c->cg_part, c->cg_state);
+        c->launches++;
+    }
+    rc = op_matvec_bead_sorted(c);
+    if (!rc) {
+        PassTimer t(c, PASS_KRYLOV);
+        k_proj_dot<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->bead.inv, c->wbead.inv, c->w_real, c->w_wave, c->kconst, c->cg_p, c->cg_t, c->cg_ap,
+                                        c->cg_part, c->cg_state);
+        k_cg_update<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->cg_p, c->cg_ap, c->cg_t, c->cg_q, c->cg_g, c->cg_psi, c->cg_part, c->cg_state,
+                                         c->cg_host_dev, pc ? 1 : 0);
+        c->launches += 2;
+        if (pc) rc = enqueue_precond(c, 0);
+    }
+    c->skip_flag = nullptr;
+    if (rc) return rc;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
+static bool graphs_enabled()
+{
+    static int on = -1;
+    if (on < 0) { const char* e = getenv("PCE_NO_GRAPH"); on = (e && e[0] == '1') ? 0 : 1; }
+    return on == 1;
+}
+
+// capture one iteration into a graph (once per system; arrays it touches are owned by the context)
+static int capture_iteration(pce_ctx* c)
+{
+    cudaGraph_t g = nullptr;
+    const long long l0 = c->launches;
+    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->cg_graph_failed = true; return PCE_OK; }
+    const int rc = enqueue_iteration(c);
+    const cudaError_t e = cudaStreamEndCapture(c->st, &g);
+    c->cg_graph_launches = c->launches - l0;
+    c->launches = l0;
+    if (rc != PCE_OK || e != cudaSuccess || !g) {
+        cudaGetLastError();
+        if (g) cudaGraphDestroy(g);
+        c->cg_graph_failed = true;  // fall back to plain launches
+        return PCE_OK;
+    }
+    if (cudaGraphInstantiate(&c->cg_graph, g, 0) != cudaSuccess) { cudaGetLastError(); c->cg_graph = nullptr; c->cg_graph_failed = true; }
+    cudaGraphDestroy(g);
+    return PCE_OK;
+}
+
+// wait (without touching the stream) until the device reports iteration `want` complete or the solve done
+static int wait_progress(pce_ctx* c, int want)
+{
+    volatile CgHostStatus* hs = c->cg_host;
+    long spins = 0;
+    while (hs->it < want && !hs->done) {
+        if ((++spins & 1023) == 0) {
+            const cudaError_t e = cudaStreamQuery(c->st);
+            if (e == cudaSuccess) {  // nothing left in the stream
+                if (hs->it < want && !hs->done) { c->err = "Krylov solve: the device stopped reporting progress"; return PCE_ECUDA; }
+            } else if (e != cudaErrorNotReady) {
+                c->err = std::string("Krylov solve: ") + cudaGetErrorString(e);
+                return PCE_ECUDA;
+            }
+        }
+    }
+    return PCE_OK;
+}
+
+// the loop shared by both systems; the state has been initialised on the device (it = 0, done, rz[0])
+static int run_iterations(pce_ctx* c, pce_solve_info* inf)
+{
+    const int maxit = c->p.max_iter;
+    int rc = PCE_OK;
+    const bool use_graph = !c->timing && graphs_enabled() && !c->cg_graph_failed;
+    if (use_graph && !c->cg_graph) {
+        if ((rc = capture_iteration(c))) return rc;
+    }
+    // iterations kept in flight: large meshes take milliseconds per iteration (an unneeded replay costs its cuFFT passes), small
+    // ones are launch-bound
+    const long long mesh = (long long)c->p.Ng[0] * c->p.Ng[1] * c->p.Ng[2];
+    const int depth = (mesh >= (1ll << 24)) ? 1 : 3;
+    int launched = 0;
+    for (;;) {
+        if (launched >= depth && (rc = wait_progress(c, launched - depth + 1))) return rc;
+        if (c->cg_host->done || launched >= maxit) break;
+        if (use_graph && c->cg_graph) {
+            PCE_CUDA(c, cudaGraphLaunch(c->cg_graph, c->st));
+            c->launches += c->cg_graph_launches;
+        } else if ((rc = enqueue_iteration(c))) return rc;
+        ++launched;
+    }
+    if ((rc = wait_progress(c, launched))) return rc;
+    inf->iters = c->cg_host->it;
+    inf->matvecs += c->cg_host->it;
+    const double gg = c->cg_host->gg, ref = c->cg_host->ref;
+    inf->rel_resid = sqrt(gg) / ref;
+    if (!(gg == gg)) { c->err = "NaN in the Krylov residual"; return PCE_ECUDA; }
+    inf->converged = (inf->rel_resid <= c->p.tol_solver) ? 1 : 0;
+    return PCE_OK;
+}
+
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi,
              pce_solve_info* info)
 {
-    const int nb = c->Nbody, nbead = c->Nbead, N = c->N;
+    const int nb = c->Nbody, nbead = c->Nbead;
     pce_solve_info inf = {0, 0, 0.0, 1};
-    // 1. starting charges
-    if (nb > 0) {
+    int rc = krylov_alloc(c);
+    if (rc) return rc;
+    // 1. starting charges (beads in the context's own iterate, ions fixed)
+    if (nb > 0 && nbead > 0) {
         PassTimer t(c, PASS_KRYLOV);
-        k_init_q<<<nb, BT, 0, c->st>>>(c->body_off, Q_body, warm, q);
-        c->launches++;
+        k_init_q<<<nb, BT, 0, c->st>>>(c->body_off, Q_body, warm, q, c->cg_q);
+        k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->cg_q, q);
+        c->launches += 2;
     }
     if (c->Nion > 0) {
         if (!q_ion) { c->err = "q_ion is NULL but the system has ions"; return PCE_EINVAL; }
@@ -239,87 +508,52 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
         return PCE_OK;
     }
     // 2. potentials of the starting charges at every bead (ions included as sources): all sources, bead targets
-    int rc = op_evaluate_at_beads(c, q, c->ev_psi);
-    if (rc) return rc;
+    if ((rc = op_evaluate_at_beads(c, q, c->cg_psi))) return rc;
     inf.matvecs = 1;
-    const int maxit = c->p.max_iter;
-    // device scalars: [0] = ref^2, [1] = |g_0|^2; iteration it: g.z at 2+3it, p.Ap at 3+3it, |g_{it+1}|^2 at 4+3it
-    double* sc = c->cg_scal;
-    double* part = c->cg_scal + 3 * (maxit + 2) + 2;  // [nb] partials
-    double* part2 = part + nb;
-    const bool pc = c->pc_on;
-    const double* zraw = pc ? c->cg_z : nullptr;
-    double* cur_rz = pc ? sc + 2 : sc + 1;
+    c->cg_host->it = -1; c->cg_host->done = 0;
     {
         PassTimer t(c, PASS_KRYLOV);
-        k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->ev_psi, c->cg_psi);
-        k_resid_init<<<nb, BT, 0, c->st>>>(c->body_off, c->rx, c->ry, c->rz, E0[0], E0[1], E0[2], c->ev_psi, c->cg_rhs, c->cg_g,
-                                         c->cg_p, part, part2);
-        c->launches += 2;
-        if ((rc = sum_to(c, part, nb, sc + 1))) return rc;
-        if ((rc = sum_to(c, part2, nb, sc + 0))) return rc;
-        if (pc) {
-            if ((rc = precond_apply(c, c->cg_g, c->cg_z))) return rc;
-            k_pc_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_z, c->cg_g, c->pc_mean, part);
-            c->launches++;
-            if ((rc = sum_to(c, part, nb, cur_rz))) return rc;
-            k_cg_pupdate<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, nullptr, nullptr, c->cg_g, zraw, c->pc_mean, c->body_of, c->cg_p);
-            c->launches++;
-        }
+        k_resid_init<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->rx, c->ry, c->rz, E0[0], E0[1], E0[2], c->cg_psi, c->cg_g, c->cg_part, c->cg_state,
+                                         c->cg_host_dev, warm, c->pc_on ? 1 : 0, c->p.tol_solver, c->p.max_iter);
+        c->launches++;
+        if (c->pc_on && (rc = enqueue_precond(c, 1))) return rc;
     }
-    double ref2 = 0.0, gg = 0.0;
-    PCE_CUDA(c, cudaMemcpyAsync(&ref2, sc + 0, sizeof(double), cudaMemcpyDeviceToHost, c->st));
-    PCE_CUDA(c, cudaMemcpyAsync(&gg, sc + 1, sizeof(double), cudaMemcpyDeviceToHost, c->st));
-    PCE_CUDA(c, cudaStreamSynchronize(c->st));
-    // Scale of the data: (|P r.E0|^2 + |P psi0|^2)^(1/2) with psi0 the potential of the uniform starting charges and the
-    // ions.  After a warm start psi0 is already nearly equipotential and that norm collapses, so the scale of the last cold
-    // solve of this system is kept and used whenever it is larger.
-    double ref = (ref2 > 0.0) ? sqrt(ref2) : 1.0;
-    if (!warm) c->cg_ref_cold = ref;
-    else if (c->cg_ref_cold > ref) ref = c->cg_ref_cold;
-    const double tol = c->p.tol_solver;
-    int it = 0;
-    inf.rel_resid = sqrt(gg) / ref;
-    while (inf.rel_resid > tol && it < maxit) {
-        double* s_pap = sc + 3 + 3 * it;
-        double* s_gn = sc + 4 + 3 * it;
-        double* next_rz = pc ? sc + 2 + 3 * (it + 1) : s_gn;
-        if ((rc = op_matvec_bead(c, c->cg_p, c->cg_t))) return rc;
-        inf.matvecs++;
-        {
-            PassTimer t(c, PASS_KRYLOV);
-            k_proj_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_t, c->cg_p, c->cg_ap, part);
-            c->launches++;
-            if ((rc = sum_to(c, part, nb, s_pap))) return rc;
-            k_cg_update<<<nb, BT, 0, c->st>>>(c->body_off, cur_rz, s_pap, c->cg_p, c->cg_ap, c->cg_t, q, c->cg_g, c->cg_psi, part);
-            c->launches++;
-            if ((rc = sum_to(c, part, nb, s_gn))) return rc;
-            PCE_CUDA(c, cudaMemcpyAsync(&gg, s_gn, sizeof(double), cudaMemcpyDeviceToHost, c->st));
-            if (pc) {
-                if ((rc = precond_apply(c, c->cg_g, c->cg_z))) return rc;
-                k_pc_dot<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_z, c->cg_g, c->pc_mean, part);
-                c->launches++;
-                if ((rc = sum_to(c, part, nb, next_rz))) return rc;
-            }
-            k_cg_pupdate<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, cur_rz, next_rz, c->cg_g, zraw, c->pc_mean, c->body_of, c->cg_p);
-            c->launches++;
-        }
-        PCE_CUDA(c, cudaStreamSynchronize(c->st));
-        cur_rz = next_rz;
-        ++it;
-        inf.rel_resid = sqrt(gg) / ref;
-        if (!(gg == gg)) { c->err = "NaN in the Krylov residual"; return PCE_ECUDA; }
-    }
-    inf.iters = it;
-    inf.converged = (inf.rel_resid <= tol) ? 1 : 0;
+    PCE_CUDA(c, cudaGetLastError());
+    if ((rc = wait_progress(c, 0))) return rc;
+    if ((rc = run_iterations(c, &inf))) return rc;
     {
         PassTimer t(c, PASS_KRYLOV);
         k_body_mean<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_psi, Phi);
-        c->launches++;
+        k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->cg_q, q);
+        c->launches += 2;
     }
     PCE_CUDA(c, cudaGetLastError());
     if (info) *info = inf;
-    (void)N;
+    return inf.converged ? PCE_OK : PCE_ENOCONV;
+}
+
+// M_bb q = b over the conductor beads, no constraint (a column of the grand capacitance tensor, eq. 15)
+int solve_plain(pce_ctx* c, const double* b, double* q, pce_solve_info* info)
+{
+    const int nbead = c->Nbead;
+    pce_solve_info inf = {0, 0, 0.0, 1};
+    int rc = krylov_alloc(c);
+    if (rc) return rc;
+    c->cg_host->it = -1; c->cg_host->done = 0;
+    {
+        PassTimer t(c, PASS_KRYLOV);
+        k_resid_init_plain<<<pupdate_blocks(c), BT, 0, c->st>>>(nbead, b, c->cg_g, c->cg_q, c->cg_psi, c->cg_part, c->cg_state, c->cg_host_dev,
+                                                               c->pc_on ? 1 : 0, c->p.tol_solver, c->p.max_iter);
+        c->launches++;
+        if (c->pc_on && (rc = enqueue_precond(c, 1))) return rc;
+    }
+    PCE_CUDA(c, cudaGetLastError());
+    if ((rc = wait_progress(c, 0))) return rc;
+    if ((rc = run_iterations(c, &inf))) return rc;
+    k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->cg_q, q);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    if (info) *info = inf;
     return inf.converged ? PCE_OK : PCE_ENOCONV;
 }
 

@@ -72,8 +72,9 @@ static void free_system(pce_ctx* c)
     cudaFree(c->csr_ptr); cudaFree(c->csr_col); cudaFree(c->csr_val);
     cudaFree(c->w_real); cudaFree(c->w_wave); cudaFree(c->w_ex); cudaFree(c->w_ey); cudaFree(c->w_ez);
     cudaFree(c->w_kx); cudaFree(c->w_ky); cudaFree(c->w_kz);
-    cudaFree(c->cg_g); cudaFree(c->cg_p); cudaFree(c->cg_t); cudaFree(c->cg_ap); cudaFree(c->cg_psi); cudaFree(c->cg_rhs);
-    cudaFree(c->ev_psi); cudaFree(c->ev_ex); cudaFree(c->ev_ey); cudaFree(c->ev_ez); cudaFree(c->cg_scal);
+    cudaFree(c->cg_g); cudaFree(c->cg_p); cudaFree(c->cg_t); cudaFree(c->cg_ap); cudaFree(c->cg_psi); cudaFree(c->cg_q);
+    cudaFree(c->ev_psi); cudaFree(c->ev_ex); cudaFree(c->ev_ey); cudaFree(c->ev_ez); cudaFree(c->cg_part);
+    krylov_invalidate_graph(c);
     cudaFree(c->hs_dev); cudaFree(c->cg_z); cudaFree(c->pc_mean);
     precond_free(c);
     c->cg_z = c->pc_mean = nullptr;
@@ -81,11 +82,12 @@ static void free_system(pce_ctx* c)
     c->rx = c->ry = c->rz = c->X = c->Y = c->Z = nullptr;
     c->csr_ptr = c->csr_col = nullptr; c->csr_val = nullptr; c->nnz = c->nnz_cap = 0;
     c->w_real = c->w_wave = c->w_ex = c->w_ey = c->w_ez = c->w_kx = c->w_ky = c->w_kz = nullptr;
-    c->cg_g = c->cg_p = c->cg_t = c->cg_ap = c->cg_psi = c->cg_rhs = nullptr;
-    c->ev_psi = c->ev_ex = c->ev_ey = c->ev_ez = c->cg_scal = nullptr;
+    c->cg_g = c->cg_p = c->cg_t = c->cg_ap = c->cg_psi = c->cg_q = nullptr;
+    c->ev_psi = c->ev_ex = c->ev_ey = c->ev_ez = c->cg_part = nullptr;
     c->hs_dev = nullptr; c->hs_dev_n = 0;
     c->have_system = false;
-    c->cg_ref_cold = 0.0;
+    if (c->cg_state) cudaMemsetAsync(c->cg_state, 0, sizeof(CgState), c->st);  // forget the residual scale of the old system
+    c->bytes = c->bytes_base;
 }
 
 extern "C" int pce_destroy(pce_ctx* c)
@@ -93,6 +95,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     if (!c) return PCE_EINVAL;
     cudaStreamSynchronize(c->st);
     free_system(c);
+    krylov_free(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
     cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
@@ -200,6 +203,7 @@ extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
     c->st = (cudaStream_t)stream;
     std::memset(&c->tm, 0, sizeof(c->tm));
     int rc = create_impl(c);
+    c->bytes_base = c->bytes;
     if (rc != PCE_OK) {
         g_create_err = c->err;
         pce_destroy(c);
@@ -288,9 +292,9 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
     ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
     ALLOC_D(c->cg_g, c->Nbead); ALLOC_D(c->cg_p, c->Nbead); ALLOC_D(c->cg_t, c->Nbead); ALLOC_D(c->cg_ap, c->Nbead);
-    ALLOC_D(c->cg_psi, c->Nbead); ALLOC_D(c->cg_rhs, c->Nbead);
+    ALLOC_D(c->cg_psi, c->Nbead); ALLOC_D(c->cg_q, c->Nbead);
     ALLOC_D(c->ev_psi, N); ALLOC_D(c->ev_ex, N); ALLOC_D(c->ev_ey, N); ALLOC_D(c->ev_ez, N);
-    ALLOC_D(c->cg_scal, 3 * (c->p.max_iter + 2) + 2 + 2 * N_body + 16);
+    ALLOC_D(c->cg_part, 3 * (N_body > 1024 ? N_body : 1024));
     ALLOC_D(c->cg_z, c->Nbead); ALLOC_D(c->pc_mean, N_body);
     c->have_system = true;
     rc = positions_impl(c, x, y, z);
@@ -398,6 +402,21 @@ static int apply_operator(pce_ctx* c, Bins& sr, Bins& sw, Bins& tr, Bins& tw, bo
     }
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
+}
+
+// the solver's operator (krylov.cu): charges already in the two sorted orders (bead.qs, wbead.qs); results stay sorted
+// (w_real, w_wave) and are assembled by the solver's projection kernel
+int op_matvec_bead_sorted(pce_ctx* c)
+{
+    c->tm.n_matvec_bead++;
+    c->tm.n_fft_pairs++;
+    c->in_bead_matvec = true;
+    int rc = real_csr_spmv(c, c->bead, c->w_real);
+    if (!rc) rc = wave_spread_bricks(c, c->wbead);
+    if (!rc) rc = wave_fft_scale_ifft(c);
+    if (!rc) rc = wave_gather_bricks(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr);
+    c->in_bead_matvec = false;
+    return rc;
 }
 
 int op_matvec_bead(pce_ctx* c, const double* q, double* psi)

@@ -66,6 +66,22 @@ struct WaveConst {
     double G[32];       // exp(-aw r^2), r = 0..P-1
 };
 
+// Device-resident state of the Krylov solve (krylov.cu): every step length, the stopping test and the iteration count live
+// here; the host only watches CgHostStatus.
+struct CgState {
+    double rz[2];        // g.z of the current iteration at [it & 1] (the previous one at the other slot)
+    double pap, gg;      // p.Ap, |g|^2
+    double psum;         // sum of the search direction (k = 0 constant of the operator, reading A1)
+    double ref, ref_cold;  // residual scale; the one of the last cold-start solve
+    double tol;
+    int it, maxit, done, project;  // project = 1: eq. 13 on the per-body-mean-projected subspace; 0: plain M q = b
+    unsigned cnt[8];     // arrival counters of the last-block-done reductions
+};
+struct CgHostStatus {
+    volatile int it, done;
+    volatile double gg, ref;
+};
+
 enum Pass { PASS_CELLS = 0, PASS_REAL, PASS_SPREAD, PASS_FFT, PASS_SCALE, PASS_IFFT, PASS_GATHER, PASS_KRYLOV, PASS_OTHER, PASS_COUNT };
 
 struct pce_ctx {
@@ -111,6 +127,7 @@ struct pce_ctx {
     double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function
     double* zshape = nullptr;  // piecewise-polynomial table of the shape factor j0(ka)^2 / k^2 as a function of k^2
     int zshape_key_lo = 0, zshape_n = 0;
+    bool zfft_attr_set = false;  // dynamic shared-memory limit of k_zfft_scale raised on this context's device
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
     int* work_ctr = nullptr;
@@ -122,10 +139,17 @@ struct pce_ctx {
     double* scal = nullptr;  // device scalars
     double* sum_part = nullptr;  // [1024] partial sums
     // Krylov vectors [Nbead]
-    double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr, *cg_rhs = nullptr;
+    double *cg_g = nullptr, *cg_p = nullptr, *cg_t = nullptr, *cg_ap = nullptr, *cg_psi = nullptr;
     double *ev_psi = nullptr, *ev_ex = nullptr, *ev_ey = nullptr, *ev_ez = nullptr;  // [N]
-    double cg_ref_cold = 0.0;   // residual scale of the last cold-start solve (see solve_cg)
-    double* cg_scal = nullptr;  // [3*(max_iter+2) + 2 + 2*Nbody + 16]
+    double* cg_q = nullptr;     // [Nbead] the iterate (copied to the caller's array when the solve ends)
+    double* cg_part = nullptr;  // [3 * max(Nbody, pupdate blocks)] per-block partials of the fixed-order sums
+    CgState* cg_state = nullptr;        // device
+    CgHostStatus* cg_host = nullptr;    // pinned, mapped: progress of the solve as the device reports it
+    CgHostStatus* cg_host_dev = nullptr;  // its device address
+    cudaGraphExec_t cg_graph = nullptr; // one captured Krylov iteration (matvec + vector kernels)
+    bool cg_graph_failed = false;
+    long long cg_graph_launches = 0;    // kernels of this library inside one replay
+    const int* skip_flag = nullptr;     // when set, the operator kernels return at once if *skip_flag != 0 (solver converged)
     // block-Jacobi preconditioner (precond.cu)
     bool pc_on = false;
     float* pc_B = nullptr;            // per-body n_i x n_i fp32 blocks
@@ -135,11 +159,14 @@ struct pce_ctx {
     long long pc_bytes = 0;
     double* cg_z = nullptr;           // [Nbead] B r before the mean is removed
     double* pc_mean = nullptr;        // [Nbody]
+    double* pc_u = nullptr;           // [Nbead] u = A^-1 1 of each body's block (0: no block)
+    double* pc_invs = nullptr;        // [Nbody] 1 / (1.u)
     // host staging for pce_step_host
     double* hs_dev = nullptr;
     size_t hs_dev_n = 0;
 
     long long bytes = 0;
+    long long bytes_base = 0;  // workspace that survives free_system (grids, plans, tables)
     long long launches = 0;
 
     // timing
@@ -225,6 +252,10 @@ int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, dou
 // krylov.cu
 int bodies_setup(pce_ctx* c);
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
+int solve_plain(pce_ctx* c, const double* b, double* q, pce_solve_info* info);  // M_bb q = b (no constraint), b and q device [Nbead]
+void krylov_free(pce_ctx* c);
+void krylov_invalidate_graph(pce_ctx* c);
+int op_matvec_bead_sorted(pce_ctx* c);  // sorted charges in bead.qs / wbead.qs -> w_real / w_wave (sorted orders)
 int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
                double* S, double* U_body, double* U_tot, double* psi_out);
 

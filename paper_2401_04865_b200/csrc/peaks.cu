@@ -68,3 +68,25 @@ extern "C" int pce_measure_fp64_peaks(double tflops[2])
     cudaFree(out);
     return cudaGetLastError() == cudaSuccess ? PCE_OK : PCE_ECUDA;
 }
+
+// ---------------------------------------------------------------- test hook: poison shared memory
+// Fills the whole dynamic shared memory of every SM with NaN bit patterns (several CTA waves of the largest size), so that a
+// kernel of this library that reads shared memory it never wrote shows up as NaN in the next result instead of passing by luck.
+__global__ void __launch_bounds__(256) k_poison_smem(int n_words, double* sink)
+{
+    extern __shared__ unsigned long long psm[];
+    for (int i = threadIdx.x; i < n_words; i += blockDim.x) psm[i] = 0x7ff8dead0000beefull;
+    __syncthreads();
+    if (sink && psm[(threadIdx.x * 7) % n_words] == 1ull) sink[0] = 1.0;  // keeps the stores alive
+}
+
+extern "C" int pce_debug_poison_shared_memory(void* stream)
+{
+    int dev = 0, nsm = 0, max_smem = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return PCE_ECUDA;
+    if (cudaFuncSetAttribute(k_poison_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess) return PCE_ECUDA;
+    k_poison_smem<<<nsm * 4, 256, (size_t)max_smem, (cudaStream_t)stream>>>(max_smem / 8, nullptr);
+    return cudaGetLastError() == cudaSuccess ? PCE_OK : PCE_ECUDA;
+}

@@ -26,6 +26,7 @@ constexpr long long PC_MAX_ELEMS = 3ll << 30;    // total fp32 storage cap: 12 G
 
 struct PcBody {          // one preconditioned body inside the current chunk
     int j0, n;           // first bead, bead count
+    int body, pad;       // body index
     long long woff;      // offset of its n x n fp64 work matrix
     long long poff;      // offset of its panels (3 x n x GJB + GJB x GJB doubles)
     long long boff;      // offset of its fp32 matrix in pc_B
@@ -191,7 +192,7 @@ k_pc_rowsum(const PcBody* __restrict__ bodies, const double* __restrict__ work, 
 
 // s_b = sum_i u_i (one CTA per body)
 __global__ void __launch_bounds__(256)
-k_pc_usum(const PcBody* __restrict__ bodies, const double* __restrict__ u, double* __restrict__ usum)
+k_pc_usum(const PcBody* __restrict__ bodies, const double* __restrict__ u, double* __restrict__ usum, double* __restrict__ inv_s_body)
 {
     __shared__ double sh[8];
     const PcBody B = bodies[blockIdx.x];
@@ -205,6 +206,7 @@ k_pc_usum(const PcBody* __restrict__ bodies, const double* __restrict__ u, doubl
         double t = 0.0;
         for (int k = 0; k < 8; ++k) t += sh[k];
         usum[blockIdx.x] = t;
+        inv_s_body[B.body] = 1.0 / t;  // kept: A^-1 r = B r + u (u.r)/s for the unconstrained solves (capacitance tensor)
     }
 }
 
@@ -238,8 +240,10 @@ struct PcRows { int j0, n, row0; int pad; long long boff; };  // CTA -> body, fi
 constexpr int PC_ROWS = 32;  // rows per CTA (4 per warp)
 
 __global__ void __launch_bounds__(256)
-k_pc_apply(const PcRows* __restrict__ rows, const float* __restrict__ Bm, const double* __restrict__ r, double* __restrict__ z)
+k_pc_apply(const PcRows* __restrict__ rows, const float* __restrict__ Bm, const double* __restrict__ r, double* __restrict__ z,
+           const int* __restrict__ skip)
 {
+    if (skip && *skip) return;  // solver already converged (krylov.cu)
     extern __shared__ double sr[];  // the body's residual
     const PcRows R = rows[blockIdx.x];
     for (int j = threadIdx.x; j < R.n; j += 256) sr[j] = r[R.j0 + j];
@@ -286,8 +290,9 @@ k_pc_apply(const PcRows* __restrict__ rows, const float* __restrict__ Bm, const 
 
 // beads of bodies without a dense block: z = r / M(0) = 4 pi eps a r
 __global__ void k_pc_identity(int n, const unsigned char* __restrict__ has_block, const int* __restrict__ body_of, double scale,
-                              const double* __restrict__ r, double* __restrict__ z)
+                              const double* __restrict__ r, double* __restrict__ z, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n && !has_block[body_of[i]]) z[i] = scale * r[i];
 }
@@ -295,8 +300,8 @@ __global__ void k_pc_identity(int n, const unsigned char* __restrict__ has_block
 // ---------------------------------------------------------------- host
 void precond_free(pce_ctx* c)
 {
-    cudaFree(c->pc_B); cudaFree(c->pc_rows); cudaFree(c->pc_has);
-    c->pc_B = nullptr; c->pc_rows = nullptr; c->pc_has = nullptr;
+    cudaFree(c->pc_B); cudaFree(c->pc_rows); cudaFree(c->pc_has); cudaFree(c->pc_u); cudaFree(c->pc_invs);
+    c->pc_B = nullptr; c->pc_rows = nullptr; c->pc_has = nullptr; c->pc_u = nullptr; c->pc_invs = nullptr;
     c->pc_on = false; c->pc_nrows_cta = 0; c->pc_max_n = 0; c->pc_bytes = 0; c->pc_nblock = 0;
 }
 
@@ -316,7 +321,7 @@ int precond_setup(pce_ctx* c)
         const int n = off[b + 1] - off[b];
         if (n < 2 || n > PC_MAX_BODY || total + (long long)n * n > PC_MAX_ELEMS) continue;
         PcBody B;
-        B.j0 = off[b]; B.n = n; B.woff = 0; B.poff = 0; B.boff = total;
+        B.j0 = off[b]; B.n = n; B.body = b; B.pad = 0; B.woff = 0; B.poff = 0; B.boff = total;
         total += (long long)n * n;
         total = (total + 3) & ~3ll;  // 16-byte aligned rows for float4 loads when n % 4 == 0
         all.push_back(B);
@@ -353,7 +358,11 @@ int precond_setup(pce_ctx* c)
     int nb_cap = 0;
     int rc = PCE_OK;
     size_t i = 0;
-    PCE_CUDA(c, cudaMalloc(&u, (size_t)c->Nbead * sizeof(double)));
+    PCE_CUDA(c, cudaMalloc(&c->pc_u, (size_t)c->Nbead * sizeof(double)));
+    PCE_CUDA(c, cudaMalloc(&c->pc_invs, (size_t)nb * sizeof(double)));
+    PCE_CUDA(c, cudaMemsetAsync(c->pc_u, 0, (size_t)c->Nbead * sizeof(double), c->st));
+    PCE_CUDA(c, cudaMemsetAsync(c->pc_invs, 0, (size_t)nb * sizeof(double), c->st));
+    u = c->pc_u;  // u = A^-1 1 per body, kept
     while (i < all.size() && rc == PCE_OK) {
         std::vector<PcBody> ch;
         long long w = 0, pz = 0;
@@ -388,13 +397,13 @@ int precond_setup(pce_ctx* c)
                 c->launches += 2;
             }
             k_pc_rowsum<<<dim3(cdiv(nmax, 8), nbz), 256, 0, c->st>>>(bp, work, u);
-            k_pc_usum<<<nbz, 256, 0, c->st>>>(bp, u, usum + b0);
+            k_pc_usum<<<nbz, 256, 0, c->st>>>(bp, u, usum + b0, c->pc_invs);
             k_pc_final<<<dim3(cdiv(nmax, 32), cdiv(nmax, 32), nbz), 256, 0, c->st>>>(bp, work, u, usum + b0, c->pc_B);
             c->launches += 3;
         }
         if (cudaStreamSynchronize(c->st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = PCE_ECUDA; c->err = "preconditioner set-up kernels failed"; }
     }
-    cudaFree(work); cudaFree(panels); cudaFree(u); cudaFree(usum); cudaFree(dbod);
+    cudaFree(work); cudaFree(panels); cudaFree(usum); cudaFree(dbod);
     if (rc == PCE_ENOMEM) {  // not enough room for the work matrices: go without
         cudaGetLastError();
         precond_free(c);
@@ -409,10 +418,10 @@ int precond_setup(pce_ctx* c)
 int precond_apply(pce_ctx* c, const double* r, double* z)
 {
     if (!c->pc_on) return PCE_OK;
-    k_pc_apply<<<c->pc_nrows_cta, 256, (size_t)c->pc_max_n * sizeof(double), c->st>>>((const PcRows*)c->pc_rows, c->pc_B, r, z);
+    k_pc_apply<<<c->pc_nrows_cta, 256, (size_t)c->pc_max_n * sizeof(double), c->st>>>((const PcRows*)c->pc_rows, c->pc_B, r, z, c->skip_flag);
     c->launches++;
     if (c->pc_nblock < c->Nbody) {
-        k_pc_identity<<<cdiv(c->Nbead, 256), 256, 0, c->st>>>(c->Nbead, c->pc_has, c->body_of, 4.0 * PCE_PI * c->p.eps_f * c->p.a, r, z);
+        k_pc_identity<<<cdiv(c->Nbead, 256), 256, 0, c->st>>>(c->Nbead, c->pc_has, c->body_of, 4.0 * PCE_PI * c->p.eps_f * c->p.a, r, z, c->skip_flag);
         c->launches++;
     }
     PCE_CUDA(c, cudaGetLastError());

@@ -456,8 +456,9 @@ int real_csr_build(pce_ctx* c, const Bins& b)
 // one warp per row; x = b.qs (sorted charges), y = psi_s (sorted)
 __global__ void __launch_bounds__(256)
 k_csr_spmv(int n, const int* __restrict__ row_ptr, const int* __restrict__ col, const double* __restrict__ val,
-           const double* __restrict__ x, double* __restrict__ y)
+           const double* __restrict__ x, double* __restrict__ y, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (row >= n) return;
@@ -473,7 +474,7 @@ int real_csr_spmv(pce_ctx* c, const Bins& b, double* psi_s)
 {
     if (b.n == 0) return PCE_OK;
     PassTimer t(c, PASS_REAL);
-    k_csr_spmv<<<cdiv((long long)b.n * 32, 256), 256, 0, c->st>>>(b.n, c->csr_ptr, c->csr_col, c->csr_val, b.qs, psi_s);
+    k_csr_spmv<<<cdiv((long long)b.n * 32, 256), 256, 0, c->st>>>(b.n, c->csr_ptr, c->csr_col, c->csr_val, b.qs, psi_s, c->skip_flag);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;

@@ -14,8 +14,9 @@
 // two divisions: ~150 fp64 instructions) and applies it to the up to four mirror points (+-ky, +-kz) of the
 // half spectrum: the pass is then bound by its 32 bytes per complex mesh point of HBM traffic, not by the fp64 pipe.
 __global__ void __launch_bounds__(256)
-k_scale(WaveConst wc, cufftDoubleComplex* __restrict__ gk)
+k_scale(WaveConst wc, cufftDoubleComplex* __restrict__ gk, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     const int nxh = wc.Nxh, ny = wc.Ng[1], nz = wc.Ng[2];
     const int hy = ny / 2 + 1, hz = nz / 2 + 1;  // iy in [0, ny/2], iz in [0, nz/2]; mirrors ny - iy, nz - iz
     const size_t total = (size_t)nxh * hy * hz;
@@ -64,7 +65,7 @@ int wave_fft_scale_ifft(pce_ctx* c)
         PassTimer t(c, PASS_SCALE);
         const size_t total = (size_t)c->wk.Nxh * (c->wk.Ng[1] / 2 + 1) * (c->wk.Ng[2] / 2 + 1);
         const int blocks = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
-        k_scale<<<blocks, 256, 0, c->st>>>(c->wk, c->gridk);
+        k_scale<<<blocks, 256, 0, c->st>>>(c->wk, c->gridk, c->skip_flag);
         c->launches++;
         PCE_CUDA(c, cudaGetLastError());
     }

@@ -275,8 +275,10 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 __global__ void __launch_bounds__(BWARPS * 32, 6)
 k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
-                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_, int* __restrict__ work_ctr)
+                const double* __restrict__ qs, double* __restrict__ grid, int vec_ok, int generic_, int* __restrict__ work_ctr,
+                const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* tab = reinterpret_cast<double*>(smem_raw);
     WarpSmem<STRIDE_PSI>* sm = reinterpret_cast<WarpSmem<STRIDE_PSI>*>(smem_raw + NTAB * sizeof(double));
@@ -300,8 +302,8 @@ k_spread_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__
         const int nh = (NH);                                                                                            \
         BRICK_WEIGHTS(false, STRIDE_PSI, BR, qs[p])                                                                     \
         for (int sb = 0; sb < nh; sb += 4) {                                                                            \
-            const bool live = sb + t < nh;                                                                              \
-            const double* w = s.wt + (sb + t) * STRIDE_PSI;                                                             \
+            const bool live = sb + t < nh;                           /* rows >= nh were never written: read row 0 */   \
+            const double* w = s.wt + (live ? sb + t : 0) * STRIDE_PSI;                                                  \
             const double bx = live ? w[g] : 0.0;                      /* B[t][g] = wx_h[x = g]            */            \
             const double ay = live ? w[BR + g] : 0.0;                 /* wy_h[y = g]                      */            \
             double wz[BR];                                            /* q_h wz_h[0..7]                   */            \
@@ -346,8 +348,9 @@ __global__ void __launch_bounds__(BWARPS * 32, FIELD ? 3 : 6)
 k_gather_bricks(WaveConst wc, int nbx, int nby, int nbz, const int* __restrict__ cell_start, WinCoefPtrs wp,
                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                 const double* __restrict__ grid, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
-                double* __restrict__ ez, int vec_ok, int generic_, int* __restrict__ work_ctr)
+                double* __restrict__ ez, int vec_ok, int generic_, int* __restrict__ work_ctr, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
     constexpr int DW = FIELD ? 2 * BR : BR;  // doubles per dimension in the weight table
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -525,7 +528,7 @@ int wave_spread_bricks(pce_ctx* c, const Bins& b)
     const int vec_ok = (c->wk.Ng[0] % 2 == 0) ? 1 : 0;
     PCE_CUDA(c, cudaMemsetAsync(c->work_ctr, 0, sizeof(int), c->st));
     k_spread_bricks<<<grid_for(c, c->occ_spread, b.ncell), BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
-                                                                                     coef_ptrs(b), b.xs, b.ys, b.zs, b.qs, c->grid, vec_ok, generic_weights(c), c->work_ctr);
+                                                                                     coef_ptrs(b), b.xs, b.ys, b.zs, b.qs, c->grid, vec_ok, generic_weights(c), c->work_ctr, c->skip_flag);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -545,11 +548,11 @@ int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, dou
         PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
         k_gather_bricks<true><<<blocks, BWARPS * 32, smem_bytes(true), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, ex_s, ey_s,
-                                                                               ez_s, vec_ok, generic_weights(c), c->work_ctr);
+                                                                               ez_s, vec_ok, generic_weights(c), c->work_ctr, c->skip_flag);
     } else {
         k_gather_bricks<false><<<blocks, BWARPS * 32, smem_bytes(false), c->st>>>(c->wk, b.nc[0], b.nc[1], b.nc[2], b.cell_start,
                                                                                  coef_ptrs(b), b.xs, b.ys, b.zs, c->grid, psi_s, nullptr,
-                                                                                 nullptr, nullptr, vec_ok, generic_weights(c), c->work_ctr);
+                                                                                 nullptr, nullptr, vec_ok, generic_weights(c), c->work_ctr, c->skip_flag);
     }
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());

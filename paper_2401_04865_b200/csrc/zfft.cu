@@ -140,8 +140,9 @@ constexpr int KP = 4;
 template <int N>
 __global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
 k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
-             const double* __restrict__ shape, int shape_key_lo)
+             const double* __restrict__ shape, int shape_key_lo, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     extern __shared__ __align__(16) unsigned char zsm[];
     double2* tile = reinterpret_cast<double2*>(zsm);       // [N][KP]
     double2* tw = tile + (size_t)N * KP;                    // [N]
@@ -207,14 +208,13 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
 template <int N> int launch(pce_ctx* c)
 {
     const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set && smem > 48 * 1024) {
+    if (!c->zfft_attr_set && smem > 48 * 1024) {  // the attribute is per device: once per context, not per process
         PCE_CUDA(c, cudaFuncSetAttribute(k_zfft_scale<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        c->zfft_attr_set = true;
     }
     const dim3 grid(cdiv(c->wk.Nxh, KP), c->wk.Ng[1] / 2 + 1);
     k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp, c->zshape,
-                                                        c->zshape_key_lo);
+                                                        c->zshape_key_lo, c->skip_flag);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;

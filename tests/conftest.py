@@ -29,3 +29,20 @@ def read_golden(path):
             k, v = line.split(None, 1)
             out[k] = float(v)
     return out
+
+
+def body_vector_error(got, want, f_oracle, floor=1e-6):
+    """Parity measure for per-body sums of bead forces (F_i, T_i: eq. 18), arrays of shape (N_body, 3).
+
+    north_star: relative L2 <= 1e-8 on forces and torques.  The plain relative L2 error |got - want| / |want| is returned
+    whenever the oracle's own norm is at least ``floor`` x the bead-force scale  max_d sum_a |f_a,d|; only when the body sums
+    vanish by symmetry (a single sphere, the ion-free lattice: |want| is rounding noise of a sum of O(1) terms) the error is
+    measured against that bead-force scale instead.  Returns (error, "rel" | "abs")."""
+    import numpy as np
+    got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
+    fscale = float(np.abs(np.asarray(f_oracle)).sum(0).max())
+    nw = float(np.linalg.norm(want))
+    d = float(np.linalg.norm(got - want))
+    if nw >= floor * fscale:
+        return d / nw, "rel"
+    return d / max(fscale, 1e-300), "abs"

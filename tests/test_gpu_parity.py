@@ -7,6 +7,7 @@ import pytest
 
 import oracle as orc
 import workloads as wl
+from conftest import body_vector_error
 
 pytestmark = pytest.mark.gpu
 
@@ -121,9 +122,10 @@ def _solve_and_compare(pce, w, tol=1e-10, P=0):
         "U_eq16": abs(float(out["U_eq16"]) - oo["U_eq16"]) / max(abs(oo["U_eq16"]), 1e-300),
         "U_MM": abs(float(out["U_MM"]) - oo["U_MM"]) / max(abs(oo["U_MM"]), 1e-300),
     }
-    fscale = np.abs(oo["f"]).sum(0).max()  # body forces/torques can vanish by symmetry: compare on the bead-force scale
-    res["F"] = float(np.abs(out["F"].cpu().numpy() - oo["F"]).max() / fscale)
-    res["T"] = float(np.abs(out["T"].cpu().numpy() - oo["T"]).max() / fscale)
+    # body forces and torques: plain relative L2 against the oracle (north_star: <= 1e-8); the bead-force scale is used only
+    # where the oracle's own |F| or |T| is below 1e-6 of it (sums that vanish by symmetry), see conftest.body_vector_error
+    res["F"], res["F_kind"] = body_vector_error(out["F"].cpu().numpy(), oo["F"], oo["f"])
+    res["T"], res["T_kind"] = body_vector_error(out["T"].cpu().numpy(), oo["T"], oo["f"])
     res["info"] = info
     res["oracle"] = oo
     res["gpu"] = out
@@ -142,11 +144,12 @@ def test_solve_config1_sphere_dipole(pce):
     assert Sz / (4 * np.pi) - 1 == pytest.approx(0.1484, abs=2e-4)  # +14.8 % at 162 beads, always larger
 
 
-@pytest.mark.parametrize("d", [2.2, 4.0])
+@pytest.mark.parametrize("d", [2.2, 4.0, 6.0])
 def test_solve_config2_two_spheres_with_ions(pce, d):
     w = wl.config2(d=d)
     r = _solve_and_compare(pce, w)
     assert r["info"]["converged"]
+    assert r["F_kind"] == "rel" and r["T_kind"] == "rel"  # true relative L2 of the (N_body, 3) arrays
     assert r["q"] < TOL_FIELD and r["psi"] < TOL_FIELD and r["Phi"] < TOL_FIELD, {k: v for k, v in r.items() if k not in ("oracle", "gpu")}
     assert r["f"] < TOL_FORCE and r["F"] < TOL_FORCE and r["T"] < TOL_FORCE and r["S"] < TOL_FIELD
     assert r["W"] < TOL_FORCE and r["U_eq16"] < TOL_FORCE and r["U_MM"] < TOL_FORCE
@@ -157,6 +160,7 @@ def test_solve_charged_bodies_tiny(pce):
     w = wl.tiny_random(seed=9, n_body=3, n_ion=30, L=6.0, Ng=32, a=0.2)
     r = _solve_and_compare(pce, w)
     assert r["q"] < TOL_FIELD and r["f"] < TOL_FORCE and r["F"] < TOL_FORCE and r["T"] < TOL_FORCE, r
+    assert r["F_kind"] == "rel" and r["T_kind"] == "rel"
     ctx, (x, y, z, Q, qi) = _ctx(pce, w)
     q, Phi, info = ctx.solve(Q, qi, w.E0)
     q2, Phi2, info2 = ctx.solve(Q, qi, w.E0, q0=q)
@@ -207,7 +211,7 @@ def test_determinism(pce):
     a = ctx.matvec(q[:w.N_bead].contiguous())
     b = ctx.matvec(q[:w.N_bead].contiguous())
     info = {"bit_identical_matvec": bool(torch.equal(a, b))}
-    # spreading uses fp64 atomics in this round: agreement to rounding, not bit-wise
+    # the spread is bit-reproducible (every mesh point written once); the gather's per-hit atomics agree to rounding
     assert rel(a.cpu().numpy(), b.cpu().numpy()) < 1e-13, info
     ctx.close()
 
@@ -362,3 +366,35 @@ def test_fused_z_pass_matches_the_3d_cufft_path(pce, Ng):
         outs.append(np.stack([t.cpu().numpy() for t in (psi, ex, ey, ez)]))
         ctx.close()
     assert rel(outs[0], outs[1]) < 1e-12, rel(outs[0], outs[1])
+
+
+def test_sparse_bricks_do_not_read_stale_shared_memory(pce):
+    """Bricks with fewer than 32 (and not a multiple of 4) hits: rows of the per-warp weight table that were never written
+    must not reach the mma operands.  Shared memory of every SM is poisoned with NaN patterns first (test hook)."""
+    w = wl.config1()  # 162 beads: every brick is sparse
+    ctx, _ = _ctx(pce, w)
+    rng = np.random.default_rng(3)
+    q = _t(rng.normal(size=w.N))
+    ref = [t.cpu().numpy() for t in ctx.evaluate(q)]
+    for _ in range(3):
+        pce.poison_shared_memory()
+        got = [t.cpu().numpy() for t in ctx.evaluate(q)]
+        pce.poison_shared_memory()
+        mv = ctx.matvec(q[:w.N_bead].contiguous()).cpu().numpy()
+        assert all(np.isfinite(g).all() for g in got) and np.isfinite(mv).all()
+        assert all(rel(g, r) < 1e-13 for g, r in zip(got, ref))
+    ctx.close()
+
+
+def test_isolated_charged_sphere_without_field_converges(pce):
+    """One charged conductor, E0 = 0, no ions: the starting potential is already almost equipotential, so the projected
+    residual scale is tiny; the solve must still stop (unprojected term of the scale) and match the oracle."""
+    w = wl.config1()
+    w.Q_body = np.array([2.5])
+    w.E0 = np.zeros(3)
+    ctx, (x, y, z, Q, qi) = _ctx(pce, w)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    assert info["converged"] and info["iters"] < 40, info
+    qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+    assert rel(q.cpu().numpy(), qo) < TOL_FIELD and abs(float(Phi[0]) - Phio[0]) < TOL_FIELD * abs(Phio[0])
+    ctx.close()

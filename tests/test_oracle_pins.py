@@ -371,3 +371,46 @@ def test_cubic_lattice_symmetry():
     q1, Phi1, _ = orc.solve_induced(w1.x, w1.body_offset, w1.Q_body, w1.q_ion, w1.E0, w1.L, w1.a)
     S1 = (orc.rel_positions(w1.x, w1.body_offset, w1.L) * q1[:, None]).sum(0)
     assert np.abs(o["S"][0] - S1).max() < 1e-11
+
+
+# ---------------------------------------------------------------- reading A7: a body across the periodic boundary
+def test_body_centres_for_a_body_across_the_periodic_boundary():
+    """X_i is the mean of the body's beads unwrapped about its first bead ("centre of mass", reading A7).
+    Translating the whole periodic system by any vector must translate X_i (mod L) and leave r_ij, the induced charges,
+    forces and torques unchanged -- also when the translation leaves the body straddling a face, an edge or a corner of
+    the box, where a naive mean of wrapped coordinates is wrong by ~L/2."""
+    w = wl.tiny_random(seed=31, n_body=2, n_ion=6, L=6.0, a=0.2)
+    off, L = w.body_offset, w.L
+    X0, r0 = orc.body_centres(w.x, off, L)
+    q0, Phi0, _ = orc.solve_induced(w.x, off, w.Q_body, w.q_ion, w.E0, L, w.a)
+    o0 = orc.forces_torques(w.x, off, q0, w.E0, L, w.a, Phi_body=Phi0)
+    c = np.asarray(w.meta["centres"])[0]
+    for shift in (np.array([0.03, 0.0, 0.0]) - [c[0], 0, 0],          # body 0 centred on the face x = 0
+                  np.array([6.0 - 0.01, 0.02, 0.0]) - [c[0], c[1], 0],  # on the edge x = L, y = 0
+                  np.array([0.01, 5.99, 0.02]) - c):                    # on a corner
+        xs = w.x + shift
+        xs -= L * np.floor(xs / L)
+        b0 = xs[off[0]:off[1]]
+        assert np.ptp(b0, axis=0).max() > 0.5 * L[0]  # the wrapped beads really sit on both sides of the box
+        X, r = orc.body_centres(xs, off, L)
+        assert np.abs(r - r0).max() < 1e-12
+        dX = X - (X0 + shift)
+        assert np.abs(dX - L * np.round(dX / L)).max() < 1e-12
+        naive = b0.mean(axis=0)  # what a mean of wrapped coordinates would give: off by a fraction of L
+        dn = naive - X[0]
+        assert np.abs(dn - L * np.round(dn / L)).max() > 0.1
+        q, Phi, _ = orc.solve_induced(xs, off, w.Q_body, w.q_ion, w.E0, L, w.a)
+        o = orc.forces_torques(xs, off, q, w.E0, L, w.a, Phi_body=Phi)
+        assert np.abs(q - q0).max() < 1e-11 * np.abs(q0).max()
+        for k in ("F", "T", "S"):
+            assert np.abs(o[k] - o0[k]).max() < 1e-10 * max(np.abs(o0["f"]).sum(0).max(), 1.0), k
+        assert np.abs(Phi - Phi0).max() < 1e-11 * max(np.abs(Phi0).max(), 1.0)
+
+
+def test_dR_small_r_branch():
+    """dR/dr for r -> 0 (the oracle's r < 1e-6 a branch and its neighbourhood): R = M_free - W with W smooth and even in r,
+    so dR/dr -> dM_free/dr = -1/(16 pi a^2) (eq. 10, reading G1), continuously through the branch point."""
+    for a, xi in ((1.0, 0.7), (0.2, 1.3), (0.0346, 1.04)):
+        lim = -1.0 / (16 * np.pi * a * a)
+        for r in (1e-9 * a, 0.5e-6 * a, 0.99e-6 * a, 1.01e-6 * a, 2e-6 * a, 1e-5 * a):
+            assert orc.dR(r, a, xi) == pytest.approx(lim, rel=2e-4), (a, xi, r)
