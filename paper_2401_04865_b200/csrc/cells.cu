@@ -110,16 +110,17 @@ int wrap_positions(pce_ctx* c, int n, const double* xi, const double* yi, const 
     return PCE_OK;
 }
 
-__global__ void k_gather_perm(int n, const int* __restrict__ perm, const double* __restrict__ in, double* __restrict__ out)
+__global__ void k_gather_perm(int n, const int* __restrict__ perm, const double* __restrict__ in, double* __restrict__ out, int stride)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) out[i] = in[perm[i]];
+    if (i < n) out[(size_t)i * stride] = in[perm[i]];
 }
 
-int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out)
+// out[i * out_stride] = in[perm[i]] (stride 16: the charge slot of the 128-byte hit records, wave_cols.cu)
+int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out, int out_stride)
 {
     if (n == 0) return PCE_OK;
-    k_gather_perm<<<cdiv(n, 256), 256, 0, c->st>>>(n, perm, in, out);
+    k_gather_perm<<<cdiv(n, 256), 256, 0, c->st>>>(n, perm, in, out, out_stride);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -246,6 +247,7 @@ void bins_free(Bins& b)
     cudaFree(b.cell_of); cudaFree(b.cell_start); cudaFree(b.cell_fill); cudaFree(b.perm); cudaFree(b.perm_tmp); cudaFree(b.inv);
     cudaFree(b.xs); cudaFree(b.ys); cudaFree(b.zs); cudaFree(b.qs);
     cudaFree(b.ws0); cudaFree(b.wcf); cudaFree(b.chunk_start);
+    wave_cols_free(b);
     b = Bins();
 }
 

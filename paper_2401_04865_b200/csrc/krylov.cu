@@ -233,7 +233,7 @@ k_pc_dot(int nb, const int* __restrict__ off, double* __restrict__ zraw, const d
 __global__ void __launch_bounds__(256)
 k_pupdate(int n, const double* __restrict__ g, const double* __restrict__ zraw, const double* __restrict__ zmean,
           const int* __restrict__ body_of, const int* __restrict__ inv_r, const int* __restrict__ inv_w, double* __restrict__ p,
-          double* __restrict__ qs_r, double* __restrict__ qs_w, double* __restrict__ part, CgState* __restrict__ st)
+          double* __restrict__ qs_r, double* __restrict__ qs_w, int qs_w_stride, double* __restrict__ part, CgState* __restrict__ st)
 {
     if (st->done) return;
     __shared__ double sh[32];
@@ -249,7 +249,7 @@ k_pupdate(int n, const double* __restrict__ g, const double* __restrict__ zraw, 
         const double v = (it > 0) ? z + beta * p[i] : z;
         p[i] = v;
         qs_r[inv_r[i]] = v;
-        qs_w[inv_w[i]] = v;
+        qs_w[(size_t)inv_w[i] * qs_w_stride] = v;
         ps += v;
     }
     ps = block_sum(ps, sh);
@@ -384,7 +384,7 @@ static int enqueue_iteration(pce_ctx* c)
     {
         PassTimer t(c, PASS_KRYLOV);
         k_pupdate<<<pupdate_blocks(c), 256, 0, c->st>>>(n, c->cg_g, pc ? c->cg_z : nullptr, c->pc_mean, c->body_of, c->bead.inv, c->wbead.inv,
-                                                        c->cg_p, c->bead.qs, c->wbead.qs, c->cg_part, c->cg_state);
+                                                        c->cg_p, c->bead.qs, c->use_cols ? c->wbead.qs_cols : c->wbead.qs, c->use_cols ? 16 : 1, c->cg_part, c->cg_state);
         c->launches++;
     }
     rc = op_matvec_bead_sorted(c);

@@ -182,6 +182,8 @@ static int create_impl(pce_ctx* c)
     cufftSetStream(c->planB, c->st);
     int rcw = wave_bricks_init(c);
     if (rcw) return rcw;
+    c->use_cols = wave_cols_supported(c);
+    if (c->use_cols && (rcw = wave_cols_init(c))) return rcw;
     return realtab_upload(c);
 }
 
@@ -241,8 +243,13 @@ static int positions_impl(pce_ctx* c, const double* x, const double* y, const do
         if ((rc = bins_build(c, c->bead, c->x, c->y, c->z))) return rc;  // beads are the first Nbead particles
         if ((rc = bins_build(c, c->wall, c->x, c->y, c->z))) return rc;
         if ((rc = bins_build(c, c->wbead, c->x, c->y, c->z))) return rc;
-        if ((rc = wave_window_coef(c, c->wall))) return rc;
-        if ((rc = wave_window_coef(c, c->wbead))) return rc;
+        if (c->use_cols) {
+            if ((rc = wave_cols_build(c, c->wall))) return rc;
+            if ((rc = wave_cols_build(c, c->wbead))) return rc;
+        } else {
+            if ((rc = wave_window_coef(c, c->wall))) return rc;
+            if ((rc = wave_window_coef(c, c->wbead))) return rc;
+        }
         if ((rc = bodies_setup(c))) return rc;
     }
     if ((rc = real_csr_build(c, c->bead))) return rc;
@@ -286,8 +293,13 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     if ((rc = bins_alloc_chunks(c, c->bead))) return rc;
     if ((rc = bins_alloc_tiles(c, c->wall, N, 8))) return rc;  // 8-point mesh bins = bricks of wave_bricks.cu
     if ((rc = bins_alloc_tiles(c, c->wbead, c->Nbead, 8))) return rc;
-    if ((rc = wave_coef_alloc(c, c->wall))) return rc;
-    if ((rc = wave_coef_alloc(c, c->wbead))) return rc;
+    if (c->use_cols) {
+        if ((rc = wave_cols_alloc(c, c->wall))) return rc;
+        if ((rc = wave_cols_alloc(c, c->wbead))) return rc;
+    } else {
+        if ((rc = wave_coef_alloc(c, c->wall))) return rc;
+        if ((rc = wave_coef_alloc(c, c->wbead))) return rc;
+    }
     PCE_CUDA(c, cudaMalloc(&c->csr_ptr, ((size_t)c->Nbead + 2) * sizeof(int)));
     ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
     ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
@@ -385,15 +397,16 @@ static int apply_operator(pce_ctx* c, Bins& sr, Bins& sw, Bins& tr, Bins& tw, bo
     {
         PassTimer t(c, PASS_OTHER);
         if ((rc = gather_by_perm(c, sr.n, sr.perm, q, sr.qs))) return rc;
-        if ((rc = gather_by_perm(c, sw.n, sw.perm, q, sw.qs))) return rc;
+        if ((rc = gather_by_perm(c, sw.n, sw.perm, q, c->use_cols ? sw.qs_cols : sw.qs, c->use_cols ? 16 : 1))) return rc;
         if ((rc = sum_vector(c, q, sr.n, c->scal))) return rc;
     }
     if (use_csr) rc = real_csr_spmv(c, sr, c->w_real);                                      // step 1 (cached), eq. 20-21
     else rc = real_direct(c, tr, sr, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);          // step 1, eq. 20-21
     if (rc) return rc;
-    if ((rc = wave_spread_bricks(c, sw))) return rc;                                      // step 2, eq. 25
+    if ((rc = c->use_cols ? wave_spread_cols(c, sw) : wave_spread_bricks(c, sw))) return rc;  // step 2, eq. 25
     if ((rc = wave_fft_scale_ifft(c))) return rc;                                        // steps 3-5, eq. 26
-    if ((rc = wave_gather_bricks(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    if ((rc = c->use_cols ? wave_gather_cols(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz)
+                          : wave_gather_bricks(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
     {
         PassTimer t(c, PASS_OTHER);
         k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, tr.inv, tw.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,
@@ -412,9 +425,10 @@ int op_matvec_bead_sorted(pce_ctx* c)
     c->tm.n_fft_pairs++;
     c->in_bead_matvec = true;
     int rc = real_csr_spmv(c, c->bead, c->w_real);
-    if (!rc) rc = wave_spread_bricks(c, c->wbead);
+    if (!rc) rc = c->use_cols ? wave_spread_cols(c, c->wbead) : wave_spread_bricks(c, c->wbead);
     if (!rc) rc = wave_fft_scale_ifft(c);
-    if (!rc) rc = wave_gather_bricks(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr);
+    if (!rc) rc = c->use_cols ? wave_gather_cols(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr)
+                              : wave_gather_bricks(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr);
     c->in_bead_matvec = false;
     return rc;
 }

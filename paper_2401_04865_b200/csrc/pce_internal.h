@@ -13,6 +13,15 @@
 
 #define PCE_PI 3.14159265358979323846
 
+// 128-byte hit record of one particle for the cached-list spread / gather (wave_cols.cu): per dimension the coefficients
+// (c0, e1, e8, 1/e8) of the exp-free window recurrence, the first support index per dimension, and the particle's charge
+struct alignas(16) HitRec {
+    double4 cf[3];
+    int4 s0;
+    double pad, q;
+};
+static_assert(sizeof(HitRec) == 128, "hit records are 128 bytes");
+
 // ---------------------------------------------------------------- binning
 // A counting-sort binning of a particle subset into a Cartesian cell grid
 // (linked-cell neighbour search).  In a dimension with fewer
@@ -41,6 +50,19 @@ struct Bins {
     // mesh binnings only: per-particle window coefficients (wave_bricks.cu, k_window_coef)
     int4* ws0 = nullptr;      // [n] first support mesh index per dimension (x, y, z, unused)
     double4* wcf = nullptr;   // [3 n] per particle and dimension: (c0, e1, e8, 1/e8), see wave_bricks.cu
+    // mesh binnings on brick-aligned meshes: cached hit lists (wave_cols.cu)
+    HitRec* hrec = nullptr;       // [n]
+    double4* wu0 = nullptr;       // [n] (u0x, u0y, u0z, -): offset of the first support point from the particle, mesh units
+    int* col_cnt = nullptr;       // [nkeys + 1] key counters (build), then the list of crowded keys
+    int* col_start = nullptr;     // [nkeys + 1] first entry of key (column, z_k)
+    int* col_ent = nullptr;       // [col_ent_cap] particle slots ordered by (column, z_k, slot)
+    int* item_start = nullptr;    // [ncell + 1] first work item of each brick (chunked binnings)
+    int2* items = nullptr;        // [col_item_cap] (brick, chunk)
+    double* col_scratch = nullptr;  // [col_item_cap][512] partial bricks of split bricks
+    int* col_arrive = nullptr;    // [ncell] arrival counters of split bricks
+    double* qs_cols = nullptr;    // &hrec[0].q: charges are written into the records (stride 16 doubles)
+    int col_chunk = 0, n_items = 0;
+    long long col_ent_cap = 0, col_item_cap = 0, nkeys = 0;
 };
 
 // real-space kernel constants (eq. 20/21)
@@ -130,6 +152,8 @@ struct pce_ctx {
     bool zfft_attr_set = false;  // dynamic shared-memory limit of k_zfft_scale raised on this context's device
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
+    bool use_cols = false;     // cached-list spread / gather (wave_cols.cu) instead of the per-call candidate walk
+    int occ_cspread = 0, occ_cgather = 0, occ_cgather_f = 0;
     int* work_ctr = nullptr;
 
     // per-call work vectors
@@ -221,7 +245,7 @@ void bins_free(Bins& b);
 int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const double* z);
 int exclusive_scan(pce_ctx* c, int* data, int n_plus_1);  // in place over n+1 entries (last input must be 0)
 int wrap_positions(pce_ctx* c, int n, const double* xi, const double* yi, const double* zi, double* xo, double* yo, double* zo);
-int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out);
+int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out, int out_stride = 1);
 
 // realspace.cu
 int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
@@ -248,6 +272,15 @@ int wave_coef_alloc(pce_ctx* c, Bins& b);
 int wave_window_coef(pce_ctx* c, const Bins& b);
 int wave_spread_bricks(pce_ctx* c, const Bins& b);
 int wave_gather_bricks(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
+
+// wave_cols.cu
+bool wave_cols_supported(const pce_ctx* c);
+int wave_cols_init(pce_ctx* c);
+int wave_cols_alloc(pce_ctx* c, Bins& b);
+void wave_cols_free(Bins& b);
+int wave_cols_build(pce_ctx* c, Bins& b);
+int wave_spread_cols(pce_ctx* c, const Bins& b);
+int wave_gather_cols(pce_ctx* c, const Bins& b, bool field, double* psi_s, double* ex_s, double* ey_s, double* ez_s);
 
 // krylov.cu
 int bodies_setup(pce_ctx* c);

@@ -15,6 +15,7 @@
 #include "pce_internal.h"
 
 #include <cmath>
+#include <cstdlib>
 
 namespace {
 
@@ -57,6 +58,37 @@ template <int R, int S> __device__ __forceinline__ void dftR(double2* v)
     else dft2<S>(v);
 }
 
+// v[r] *= w^r, w = exp(S 2 pi i tstep / N) (table tw[m] = exp(-2 pi i m / N)), then the radix-R butterfly
+template <int R, int S>
+__device__ __forceinline__ void twiddle_dft(double2* v, int tstep, const double2* __restrict__ tw)
+{
+    if (tstep != 0) {
+        // w, w^2, w^4 from the table (three loads instead of seven: threads of a warp read different k, i.e. conflicting
+        // banks), the rest by products
+        double2 w1 = tw[tstep];
+        if (S > 0) w1.y = -w1.y;
+        if (R == 2) {
+            v[1] = cmul(v[1], w1);
+        } else {
+            double2 w2 = tw[2 * tstep];
+            if (S > 0) w2.y = -w2.y;
+            const double2 w3 = cmul(w1, w2);
+            v[1] = cmul(v[1], w1);
+            v[2] = cmul(v[2], w2);
+            v[3] = cmul(v[3], w3);
+            if (R == 8) {
+                double2 w4 = tw[4 * tstep];
+                if (S > 0) w4.y = -w4.y;
+                v[4] = cmul(v[4], w4);
+                v[5] = cmul(v[5], cmul(w4, w1));
+                v[6] = cmul(v[6], cmul(w4, w2));
+                v[7] = cmul(v[7], cmul(w4, w3));
+            }
+        }
+    }
+    dftR<R, S>(v);
+}
+
 // One Stockham stage of radix R on the thread's 8 elements (8/R butterflies).  in/out: element i of the pencil at
 // base[i * stride].  Loads (with the optional per-element scale g, radix 8 only), barrier if in place, stores.
 template <int N, int R, int S, bool SYNC>
@@ -81,32 +113,7 @@ __device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok
     for (int q = 0; q < NB; ++q) {
         const int b = j + q * NT;
         const int k = b & (Ns - 1);
-        const int tstep = k * (N / (Ns * R));
-        if (tstep != 0) {
-            // twiddles w^r, w = exp(S 2 pi i k / (Ns R)): w, w^2, w^4 from the table (three loads instead of seven: threads of
-            // a warp read different k, i.e. conflicting banks), the rest by products
-            double2 w1 = tw[tstep];
-            if (S > 0) w1.y = -w1.y;
-            if (R == 2) {
-                v[q * R + 1] = cmul(v[q * R + 1], w1);
-            } else {
-                double2 w2 = tw[2 * tstep];
-                if (S > 0) w2.y = -w2.y;
-                const double2 w3 = cmul(w1, w2);
-                v[q * R + 1] = cmul(v[q * R + 1], w1);
-                v[q * R + 2] = cmul(v[q * R + 2], w2);
-                v[q * R + 3] = cmul(v[q * R + 3], w3);
-                if (R == 8) {
-                    double2 w4 = tw[4 * tstep];
-                    if (S > 0) w4.y = -w4.y;
-                    v[q * R + 4] = cmul(v[q * R + 4], w4);
-                    v[q * R + 5] = cmul(v[q * R + 5], cmul(w4, w1));
-                    v[q * R + 6] = cmul(v[q * R + 6], cmul(w4, w2));
-                    v[q * R + 7] = cmul(v[q * R + 7], cmul(w4, w3));
-                }
-            }
-        }
-        dftR<R, S>(v + q * R);
+        twiddle_dft<R, S>(v + q * R, k * (N / (Ns * R)), tw);
         const int d = (b - k) * R + k;
 #pragma unroll
         for (int r = 0; r < R; ++r)
@@ -205,6 +212,155 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
     }
 }
 
+
+// ---------------------------------------------------------------- pipelined variant (N_z = 64 ... 1024 with N = 8^m * rest)
+// Same arithmetic, arranged so that HBM is kept busy: persistent CTAs walk (k_x tile, |k_y|) pairs; the [N_z][KP] tile of the
+// NEXT row streams into a second shared-memory buffer with cp.async while the current row runs its stages; the last forward
+// stage, the multiplication by the Green's function and the first inverse stage are one register-resident step (the last
+// forward stage of radix R leaves element b + r N/R in slot r, which is exactly what the first inverse stage of radix R reads),
+// so a row costs 2 fewer shared-memory passes and 3 fewer barriers.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+
+template <int N>
+__global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 2 : 1)
+k_zfft_scale_pipe(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
+                  const double* __restrict__ shape, int shape_key_lo, const int* __restrict__ skip)
+{
+    if (skip && *skip) return;
+    constexpr int REST = Radices<N>::rest, N8 = Radices<N>::n8;   // N = 8^N8 * REST (REST = 8 counts as one more radix-8 stage)
+    constexpr int NT = N / 8 * KP;
+    extern __shared__ __align__(16) unsigned char zsm[];
+    double2* tile0 = reinterpret_cast<double2*>(zsm);        // [2][N][KP]
+    double2* tw = tile0 + (size_t)2 * N * KP;                 // [N]
+    double* gs = reinterpret_cast<double*>(tw + N);           // [N][KP]
+    const int tid = threadIdx.x, p = tid % KP, j = tid / KP;
+    for (int i = tid; i < N; i += NT) tw[i] = tw_g[i];
+    const int nxh = wc.Nxh, ny = wc.Ng[1];
+    const int ntx = (nxh + KP - 1) / KP, nyh = ny / 2 + 1;
+    const int npairs = ntx * nyh;
+    const size_t zstr = (size_t)ny * nxh;
+    // rows of this CTA, flattened: pair = blockIdx.x + m gridDim.x, pass 0 (row iy) and, unless self-mirrored, pass 1 (row ny - iy)
+    auto row_of = [&](int pair, int pass, int& y, int& tx) {
+        tx = pair % ntx;
+        const int iy = pair / ntx;
+        y = (pass == 0) ? iy : ((iy == 0 || 2 * iy == ny) ? -1 : ny - iy);
+    };
+    auto issue = [&](int pair, int pass, double2* buf) {  // cp.async of one row tile; columns beyond N_x/2 re-read the last one
+        int y, tx;
+        row_of(pair, pass, y, tx);
+        const int kx = min(tx * KP + p, nxh - 1);
+        const double2* col = gk + (size_t)y * nxh + kx;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int z = j + r * (N / 8);
+            cp_async16(buf + z * KP + p, col + (size_t)z * zstr);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int pair = blockIdx.x, pass = 0, cur = 0;
+    if (pair >= npairs) return;
+    issue(pair, 0, tile0);
+    while (pair < npairs) {
+        // the row after this one
+        int npair = pair, npass = pass + 1;
+        {
+            int y1, tx1;
+            if (npass == 1) row_of(pair, 1, y1, tx1);
+            if (npass == 2 || y1 < 0) { npair = pair + gridDim.x; npass = 0; }
+        }
+        double2* sp_tile = tile0 + (size_t)cur * N * KP;
+        __syncthreads();  // the other buffer (previous row) and the Green's function table are free again
+        if (npair < npairs) issue(npair, npass, tile0 + (size_t)(cur ^ 1) * N * KP);
+        int y, tx;
+        row_of(pair, pass, y, tx);
+        if (pass == 0) {  // Green's function of the pair (even in k_y and k_z): N/2 + 1 evaluations per pencil
+            const int iy = pair / ntx;
+            const double ky = wc.kfac[1] * iy;
+            const double* ez = zexp + nxh + ny / 2 + 1;
+            for (int e = tid; e < (N / 2 + 1) * KP; e += NT) {
+                const int iz = e / KP, pp = e % KP, kxe = tx * KP + pp;
+                double f = 0.0;  // k = 0 removed; pencils beyond N_x/2 unused
+                if (kxe < nxh) {
+                    const double kx = wc.kfac[0] * kxe, kz = wc.kfac[2] * (double)iz;
+                    const double k2 = kx * kx + ky * ky + kz * kz;
+                    if (k2 > 0.0) f = wc.scale_norm * zexp[kxe] * zexp[nxh + iy] * ez[iz] * shape_eval(shape, shape_key_lo, k2);
+                }
+                gs[iz * KP + pp] = f;
+                if (iz > 0 && iz < N / 2) gs[(N - iz) * KP + pp] = f;
+            }
+        }
+        if (npair < npairs) asm volatile("cp.async.wait_group 1;" ::: "memory");
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+        const int kxi = tx * KP + p;
+        const bool col_ok = kxi < nxh;
+        double2* col = gk + (size_t)y * nxh + (col_ok ? kxi : 0);
+        double2* sp = sp_tile + p;
+        // ---- forward: all radix-8 stages but the last stage of the transform, in place
+        int Ns = 1;
+        constexpr int NF8 = (REST == 8) ? N8 - 1 : N8;  // radix-8 stages before the fused one
+        if (NF8 >= 1) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        // ---- last forward stage (radix REST, Ns = N / REST) x Green's function x first inverse stage (radix REST, Ns = 1)
+        {
+            constexpr int R = REST, NB = 8 / R, NTH = N / 8;
+            double2 v[8];
+#pragma unroll
+            for (int q = 0; q < NB; ++q) {
+                const int b = j + q * NTH;
+#pragma unroll
+                for (int r = 0; r < R; ++r) v[q * R + r] = sp[(size_t)(b + r * (N / R)) * KP];
+            }
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < NB; ++q) {
+                const int b = j + q * NTH;  // b < N / R = Ns: k = b, twiddle step k N / (Ns R) = b
+                twiddle_dft<R, -1>(v + q * R, b, tw);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const double gf = gs[(b + r * (N / R)) * KP + p];
+                    v[q * R + r].x *= gf; v[q * R + r].y *= gf;
+                }
+                dftR<R, +1>(v + q * R);  // Ns = 1: no twiddles; outputs at b R + r
+#pragma unroll
+                for (int r = 0; r < R; ++r) sp[(size_t)(b * R + r) * KP] = v[q * R + r];
+            }
+            __syncthreads();
+        }
+        // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
+        Ns = REST;
+        if (NF8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (NF8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
+        pair = npair; pass = npass; cur ^= 1;
+    }
+}
+
+template <int N> int launch_pipe(pce_ctx* c)
+{
+    const size_t smem = (size_t)2 * N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
+    if (!c->zfft_attr_set) {
+        PCE_CUDA(c, cudaFuncSetAttribute(k_zfft_scale_pipe<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->zfft_attr_set = true;
+    }
+    const int npairs = cdiv(c->wk.Nxh, KP) * (c->wk.Ng[1] / 2 + 1);
+    int per_sm = (int)((220 * 1024) / (smem + 1024));
+    if (per_sm > 2) per_sm = 2;
+    if (per_sm < 1) per_sm = 1;
+    int blocks = c->num_sm * per_sm;
+    if (blocks > npairs) blocks = npairs;
+    k_zfft_scale_pipe<N><<<blocks, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp, c->zshape,
+                                                             c->zshape_key_lo, c->skip_flag);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
 template <int N> int launch(pce_ctx* c)
 {
     const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
@@ -268,6 +424,17 @@ int zfft_init(pce_ctx* c)
 
 int zfft_scale(pce_ctx* c)
 {
+    static const bool no_pipe = [] { const char* e = getenv("PCE_ZFFT_PIPE"); return e && e[0] == '0'; }();
+    if (!no_pipe) {  // pipelined variant: meshes with at least two radix stages
+        switch (c->p.Ng[2]) {
+            case 64: return launch_pipe<64>(c);
+            case 128: return launch_pipe<128>(c);
+            case 256: return launch_pipe<256>(c);
+            case 512: return launch_pipe<512>(c);
+            case 1024: return launch_pipe<1024>(c);
+            default: break;
+        }
+    }
     switch (c->p.Ng[2]) {
         case 16: return launch<16>(c);
         case 32: return launch<32>(c);

@@ -398,3 +398,27 @@ def test_isolated_charged_sphere_without_field_converges(pce):
     qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
     assert rel(q.cpu().numpy(), qo) < TOL_FIELD and abs(float(Phi[0]) - Phio[0]) < TOL_FIELD * abs(Phio[0])
     ctx.close()
+
+
+@pytest.mark.parametrize("cfg", ["tiny", "cfg2", "cfg3"])
+def test_cached_list_spread_gather_matches_the_walk_kernels(pce, cfg, monkeypatch):
+    """Brick-aligned meshes use cached per-column hit lists (wave_cols.cu: records prefetched with cp.async, dead planes
+    skipped, crowded bricks split into chunks on small meshes); PCE_NO_COLS=1 selects the per-call candidate walk of
+    wave_bricks.cu instead.  Same window, same bricks: the two must agree to rounding, and the cached-list spread must be
+    bit-reproducible from call to call."""
+    import torch
+    w = {"tiny": lambda: wl.tiny_random(seed=17, n_body=2, n_ion=40, L=6.0, Ng=32, a=0.2, neutral=False),
+         "cfg2": lambda: wl.config2(d=2.5), "cfg3": wl.config3}[cfg]()
+    rng = np.random.default_rng(8)
+    q = _t(rng.normal(size=w.N))
+    outs = []
+    for no_cols in ("0", "1"):
+        monkeypatch.setenv("PCE_NO_COLS", no_cols)
+        ctx, _ = _ctx(pce, w)
+        full = torch.stack(ctx.evaluate(q))
+        mv = ctx.matvec(q[:w.N_bead].contiguous())
+        mv2 = ctx.matvec(q[:w.N_bead].contiguous())
+        assert rel(mv2.cpu().numpy(), mv.cpu().numpy()) < 1e-13
+        outs.append((full.cpu().numpy(), mv.cpu().numpy()))
+        ctx.close()
+    assert rel(outs[0][0], outs[1][0]) < 1e-12 and rel(outs[0][1], outs[1][1]) < 1e-12
