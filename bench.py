@@ -1,10 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the whole hot path on synthetic inputs.
 
-One "step" = cell lists + cached near field, the induced-charge Krylov solve (eq. 13), the final
-potential+field evaluation, forces / torques / energies -- i.e. set_positions + solve + forces through the
-C ABI.  metric = Ewald operator applications per second over whole steps (bead-only solver matvecs plus full
-evaluations), ms_per_step = induced-charge solve ms/step (BASELINE.json's two headline numbers).
+One "step" = cell lists + cached near field + cached spread/gather lists, the induced-charge Krylov solve (eq. 13), the
+final potential+field evaluation, forces / torques / energies -- i.e. set_positions + solve + forces through the C ABI.
+metric = Ewald operator applications per second over whole steps; the two flavours differ 3-12x in work and are also
+reported separately: M1 = bead-only solver matvec (psi at the conductor beads), M2 = full evaluation (all particles; psi
+for the right-hand side, psi + E for the forces).  ms_per_step = whole step; solve.solve_ms_per_step = the Krylov solve
+alone (BASELINE.json's second headline number).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
@@ -58,6 +60,18 @@ def make_workload(idx, rank=0):
     if idx == 4:
         return wl.config4(seed=seed)
     return wl.config5(seed=seed)
+
+
+def config_dict(w, args):
+    """The `config` object of the JSON line: the workload and the Ewald parameters that follow from it (pure host arithmetic,
+    pce_suggest_params), identical in both arms so that the driver can pair them."""
+    import paper_2401_04865_b200 as pce
+    prm = pce.suggest_params(w.L, w.Ng, w.a, args.tol, args.P)
+    grid_bytes = 8 * int(np.prod(w.Ng))
+    return {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "N_body": w.N_body, "grid": [int(g) for g in w.Ng],
+            "P": int(prm.P), "xi": prm.xi, "rc": prm.rc, "ewald_tol": args.tol, "solver_tol": args.tol_solver,
+            "l2": "flushed between timed steps" if grid_bytes < 256 << 20 else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
+            "multi_gpu": "replicas only"}
 
 
 def peaks():
@@ -175,8 +189,10 @@ def run_reference(args, rank, world):
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "grid": [int(g) for g in w.Ng]},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": desc},
+        "dtype": "f64", "data": "synthetic", "config": config_dict(w, args),
+        "counts": "one direct-sum M1 application (bead sources and targets, potential only) per step",
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                         "sample": "direct-sum oracle, " + desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
@@ -274,6 +290,28 @@ def run_ours(args, rank, world, local_rank):
     total_ms, n_apply_all = reduce_over_ranks(dist, total_ms, n_apply, "cuda")
     value = n_apply_all / (total_ms * 1e-3)
 
+    # ---- the two operator flavours on their own (CUDA events around back-to-back applications, this stream)
+    def time_op(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+    flavours = {}
+    reps = 10 if w.N > 100000 else 50
+    if w.N_bead:
+        qb = torch.randn(w.N_bead, dtype=torch.float64, device="cuda")
+        ms1 = time_op(lambda: ctx.matvec(qb), reps)
+        flavours["m1_bead_matvec"] = {"ms": ms1, "per_s": 1e3 / ms1, "what": "psi = M_bb q at the conductor beads (cached near field + spread/FFT/scale/IFFT/gather)"}
+    qa = torch.randn(w.N, dtype=torch.float64, device="cuda")
+    ms2 = time_op(lambda: ctx.evaluate(qa, field=True), max(reps // 5, 2))
+    flavours["m2_full_evaluation"] = {"ms": ms2, "per_s": 1e3 / ms2, "what": "psi and E at all N particles from all N charges"}
+    flavours["per_step"] = {"m1": float(np.mean(iters)), "m2": 2.0}
+
     # ---- end to end through the host-buffer call (H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -345,7 +383,8 @@ def run_ours(args, rank, world, local_rank):
     dom = max(own, key=lambda k: own[k]["ms_per_launch"] * own[k]["launches"])
     roof = dict(own[dom])
     roof["kernel"] = dom
-    roof["peak_source"] = peak_src
+    roof["peak_source"] = ("pce_measure_fp64_peaks (csrc/peaks.cu: fp64 mma.sync chains on this device, this run)" if roof["bound"] == "alu"
+                           else peak_src)
     roof["traffic"] = None  # dram bytes per launch from the committed ncu --set full capture (config 5 only)
     tpath = os.path.join(ROOT, "profiles", "r1f_traffic.json")
     if args.config == 5 and os.path.exists(tpath):
@@ -354,13 +393,12 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "N_body": w.N_body, "grid": [int(g) for g in w.Ng],
-                   "P": int(ctx.params.P), "xi": ctx.params.xi, "rc": ctx.params.rc, "ewald_tol": args.tol,
-                   "solver_tol": args.tol_solver, "cells": info["ncell"], "nnz_near": info["nnz_near"],
-                   "l2": "flushed between timed steps" if l2_flush is not None else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
-                   "fft": "cuFFT 2-D D2Z/Z2D per mesh plane; the 'scale' pass is the fused z FFT + Green's function + inverse z FFT kernel"
-                          if int(w.Ng[2]) in (16, 32, 64, 128, 256, 512, 1024) else "cuFFT 3-D D2Z/Z2D + separate scale pass",
-                   "multi_gpu": "replicas only"},
+        "config": config_dict(w, args),
+        "run_info": {"cells": info["ncell"], "nnz_near": info["nnz_near"],
+                     "fft": "cuFFT 2-D D2Z/Z2D per mesh plane; the 'scale' pass is the fused z FFT + Green's function + inverse z FFT kernel"
+                            if int(w.Ng[2]) in (16, 32, 64, 128, 256, 512, 1024) else "cuFFT 3-D D2Z/Z2D + separate scale pass"},
+        "counts": "value = (M1 bead-only solver matvecs + M2 full evaluations) / whole-step time; the flavours are split in 'flavours'",
+        "flavours": flavours,
         "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
                   "evals_full": acc["n_eval_full"], "rel_resid": sinfo["rel_resid"], "converged": sinfo["converged"]},
         "passes_ms_per_step": {k: acc[k] / args.steps for k in ("cells", "real", "spread", "fft", "scale", "ifft", "gather", "krylov", "other", "total")},

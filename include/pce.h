@@ -174,6 +174,24 @@ int pce_forces(pce_ctx* ctx, const double* q, const double E0[3],
                double* fx, double* fy, double* fz,
                double* F, double* T, double* S, double* U_body, double* U_tot, double* psi);
 
+/* Grand capacitance tensor of the conductor bodies, C = Sigma' M^-1 Sigma'^T (eq. 15):
+ *   [Q; S] = C [Psi - Psi_0; E_0],  blocks as in eq. 37.
+ * M is the bead-bead potential tensor (eq. 9) of the N_bead conductor beads; ions are not conductors and are left out.
+ * Index convention (Sigma' of the Appendix): k < N_body = potential / charge of body k;
+ * k = N_body + 3 i + d = field / dipole component d of body i.  For every requested column k the SPD system
+ * M_bb q = Sigma'^T e_k is solved on the device (conjugate gradients, preconditioned by the inverse of every body's own
+ * free-space tensor) and its moments Sigma' q are returned.
+ *  cols : host int[ncol], each in [0, 4 N_body);  C : device [ncol][4 N_body], row j = column cols[j] of C.
+ * info (may be NULL): worst iteration count / residual over the columns, total matvecs.  PCE_ENOCONV if any column hit max_iter. */
+int pce_capacitance_columns(pce_ctx* ctx, int ncol, const int* cols, double* C, pce_solve_info* info);
+
+/* Effective permittivity tensor of the (periodic) dispersion, eq. 36:
+ *   eps_eff = eps_f - n < C_SPsi C_qPsi^-1 C_qE - C_SE >,  n = N_body / V.
+ * The bracket is the mean dipole response of floating bodies (Q = 0) to a field common to all bodies, so it is computed by
+ * three constrained solves of eq. 13 with E0 = e_x, e_y, e_z, Q = 0 and no ionic charge (3 solves instead of 4 N_body
+ * columns); the oracle evaluates eq. 36 from the blocks of C literally.  eps_eff: host [9], row-major. */
+int pce_effective_permittivity(pce_ctx* ctx, double eps_eff[9], pce_solve_info* info);
+
 /* One whole pass of the hot path from HOST buffers (what bench.py's "e2e"
  * times): copy positions and charges to the device, rebuild cells, solve
  * eq. 13, evaluate forces, copy results back.  All pointers host; x,y,z [N];

@@ -7,5 +7,5 @@ from there.
 """
 from .oracle import (  # noqa: F401
     build, M_free, R, R0, dR, ewald_eval, pair_matrix, body_centres, rel_positions,
-    solve_induced, forces_torques, default_xi, num_threads,
+    solve_induced, forces_torques, default_xi, num_threads, sigma_prime, capacitance, effective_permittivity,
 )

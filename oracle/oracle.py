@@ -284,3 +284,42 @@ def forces_torques(x, body_offset, q, E0, L, a, eps=1.0, Phi_body=None, xi=None,
     out.update(U_body=np.concatenate([U_body, U_ion]), U_eq16=float(U_body.sum() + U_ion.sum()),
                Phi_body=Phi_body)
     return out
+
+
+# ---------------------------------------------------------------- grand capacitance tensor (eq. 15) and eps_eff (eq. 36)
+def sigma_prime(x, body_offset, L):
+    """Sigma' (Appendix eq. 52-53): the 4 N_body x N_bead summation tensor whose first N_body rows are
+    Sigma (consecutive ones over the beads of each body) and whose next 3 N_body rows carry r_ij in place of the ones;
+    row N_body + 3 i + d holds component d of r_ij for body i."""
+    off = np.asarray(body_offset, dtype=np.int64)
+    nb, nbead = len(off) - 1, int(off[-1])
+    _, r = body_centres(x, off, L)
+    Sp = np.zeros((4 * nb, nbead))
+    for i in range(nb):
+        sl = slice(off[i], off[i + 1])
+        Sp[i, sl] = 1.0
+        for d in range(3):
+            Sp[nb + 3 * i + d, sl] = r[sl, d]
+    return Sp
+
+
+def capacitance(x, body_offset, L, a, eps=1.0, s=6.0):
+    """Grand capacitance tensor C = Sigma' M^-1 Sigma'^T (eq. 15) of the conductor bodies, dense:
+    [Q; S] = C [Psi - Psi_0; E_0].  M is the bead-bead potential tensor (eq. 9) of the N_bead beads alone (ions are not
+    conductors and carry no unknowns).  Returns the 4 N_body x 4 N_body matrix, blocks as in eq. 37:
+    C[:nb, :nb] = C_qPsi, C[:nb, nb:] = C_qE, C[nb:, :nb] = C_SPsi, C[nb:, nb:] = C_SE."""
+    off = np.asarray(body_offset, dtype=np.int64)
+    nbead = int(off[-1])
+    M = pair_matrix(np.asarray(x, dtype=np.float64)[:nbead], L, a, eps, s=s)
+    Sp = sigma_prime(x, off, L)
+    return Sp @ np.linalg.solve(M, Sp.T)
+
+
+def effective_permittivity(C, n_body, V, eps=1.0):
+    """eq. 36: eps_eff = eps_f - n <C_SPsi C_qPsi^-1 C_qE - C_SE>, n = N_body / V, with <.> the average over
+    the bodies of the response to a field that is the same on every body: <X> = (1/N_b) sum_ij X_ij (3 x 3 blocks)."""
+    nb = n_body
+    Cq, CqE, CS, CSE = C[:nb, :nb], C[:nb, nb:], C[nb:, :nb], C[nb:, nb:]
+    X = CS @ np.linalg.solve(Cq, CqE) - CSE          # (3 nb) x (3 nb)
+    avg = X.reshape(nb, 3, nb, 3).sum(axis=(0, 2)) / nb
+    return eps * np.eye(3) - (nb / V) * avg

@@ -22,6 +22,7 @@ EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
     "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks", "pce_debug_poison_shared_memory",
+    "pce_capacitance_columns", "pce_effective_permittivity",
 )
 
 
@@ -89,6 +90,8 @@ def load():
     lib.pce_launch_count.restype = C.c_longlong
     lib.pce_measure_fp64_peaks.argtypes = [C.POINTER(C.c_double)]
     lib.pce_debug_poison_shared_memory.argtypes = [vp]
+    lib.pce_capacitance_columns.argtypes = [vp, C.c_int, ip, vp, C.POINTER(PceSolveInfo)]
+    lib.pce_effective_permittivity.argtypes = [vp, dp, C.POINTER(PceSolveInfo)]
     lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
@@ -243,6 +246,23 @@ class Context:
                                      _ptr(Ub), _ptr(Ut), _ptr(psi)))
         return {"f": self.torch.stack(f, dim=1), "F": F.view(3, nb).T, "T": T.view(3, nb).T, "S": S.view(3, nb).T,
                 "U_body": Ub, "U_eq16": Ut[0], "W": Ut[1], "U_MM": Ut[2], "psi": psi}
+
+    def capacitance_columns(self, cols):
+        """Columns of C = Sigma' M^-1 Sigma'^T (eq. 15): tensor [len(cols), 4 N_body]."""
+        cols = np.ascontiguousarray(cols, dtype=np.int32)
+        out = self._new(len(cols) * 4 * self.N_body)
+        info = PceSolveInfo()
+        self._ck(self.lib.pce_capacitance_columns(self.h, len(cols), cols.ctypes.data_as(C.POINTER(C.c_int)), _ptr(out), C.byref(info)))
+        return out.view(len(cols), 4 * self.N_body), {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid,
+                                                        "converged": bool(info.converged)}
+
+    def effective_permittivity(self):
+        """eps_eff (3 x 3 numpy array), eq. 36."""
+        out = (C.c_double * 9)()
+        info = PceSolveInfo()
+        self._ck(self.lib.pce_effective_permittivity(self.h, out, C.byref(info)))
+        return np.array(list(out)).reshape(3, 3), {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid,
+                                                    "converged": bool(info.converged)}
 
     def step_host(self, x, y, z, Q_body, q_ion, E0, out):
         """Host-buffer pass.  x,y,z,Q_body,q_ion: host numpy/pinned-torch f64; ``out``: dict of host arrays

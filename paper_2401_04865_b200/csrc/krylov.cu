@@ -668,3 +668,100 @@ int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, doub
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
 }
+
+// ---------------------------------------------------------------- grand capacitance tensor (eq. 15) and eps_eff (eq. 36)
+// right-hand side Sigma'^T e_k: column k < N_body: 1 on the beads of body k; column N_body + 3 i + d: r_ij,d on the beads of body i
+__global__ void k_cap_rhs(int n, int nb, int col, const int* __restrict__ body_of, const double* __restrict__ rx, const double* __restrict__ ry,
+                          const double* __restrict__ rz, double* __restrict__ b)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const int body = body_of[j];
+    double v = 0.0;
+    if (col < nb) v = (body == col) ? 1.0 : 0.0;
+    else {
+        const int i = (col - nb) / 3, d = (col - nb) % 3;
+        if (body == i) v = (d == 0) ? rx[j] : (d == 1) ? ry[j] : rz[j];
+    }
+    b[j] = v;
+}
+
+// moments [Q; S] = Sigma' q: out[i] = sum_j q_ij, out[nb + 3 i + d] = sum_j r_ij,d q_ij (one CTA per body, fixed order)
+__global__ void __launch_bounds__(BT)
+k_cap_moments(int nb, const int* __restrict__ off, const double* __restrict__ q, const double* __restrict__ rx, const double* __restrict__ ry,
+              const double* __restrict__ rz, double* __restrict__ out)
+{
+    __shared__ double sh[32];
+    const int b = blockIdx.x;
+    const int j0 = off[b], j1 = off[b + 1];
+    double a[4] = {0, 0, 0, 0};
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        const double qj = q[j];
+        a[0] += qj; a[1] += rx[j] * qj; a[2] += ry[j] * qj; a[3] += rz[j] * qj;
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) a[k] = block_sum(a[k], sh);
+    if (threadIdx.x == 0) { out[b] = a[0]; out[nb + 3 * b] = a[1]; out[nb + 3 * b + 1] = a[2]; out[nb + 3 * b + 2] = a[3]; }
+}
+
+int capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_solve_info* info)
+{
+    const int nb = c->Nbody, n = c->Nbead;
+    pce_solve_info worst = {0, 0, 0.0, 1};
+    int rc_all = PCE_OK;
+    for (int k = 0; k < ncol; ++k) {
+        const int col = cols[k];
+        if (col < 0 || col >= 4 * nb) { c->err = "pce_capacitance_columns: column index out of range"; return PCE_EINVAL; }
+        double *b = c->ev_psi, *q = c->ev_ex;  // the evaluation work vectors are free between operator calls
+        k_cap_rhs<<<cdiv(n, 256), 256, 0, c->st>>>(n, nb, col, c->body_of, c->rx, c->ry, c->rz, b);
+        c->launches++;
+        pce_solve_info inf;
+        int rc = solve_plain(c, b, q, &inf);
+        if (rc != PCE_OK && rc != PCE_ENOCONV) return rc;
+        if (rc == PCE_ENOCONV) rc_all = PCE_ENOCONV;
+        k_cap_moments<<<nb, BT, 0, c->st>>>(nb, c->body_off, q, c->rx, c->ry, c->rz, C + (size_t)k * 4 * nb);
+        c->launches++;
+        worst.iters = worst.iters > inf.iters ? worst.iters : inf.iters;
+        worst.matvecs += inf.matvecs;
+        worst.rel_resid = worst.rel_resid > inf.rel_resid ? worst.rel_resid : inf.rel_resid;
+        worst.converged = worst.converged && inf.converged;
+    }
+    PCE_CUDA(c, cudaGetLastError());
+    if (info) *info = worst;
+    return rc_all;
+}
+
+// eq. 36: eps_eff = eps_f - n <C_SPsi C_qPsi^-1 C_qE - C_SE>.  The bracket is the mean dipole response of
+// floating bodies (Q = 0: the potentials adjust) to a unit field that is the same on every body, i.e. the constrained solve
+// of eq. 13 with E0 = e_d, Q = 0 and no ionic charge: column d of eps_eff - eps_f I is (1/V) sum_i S_i.
+int effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info)
+{
+    const int nb = c->Nbody, N = c->N;
+    pce_solve_info worst = {0, 0, 0.0, 1};
+    int rc_all = PCE_OK;
+    double *zeros = c->ev_ey, *q = c->ev_ez, *Phi = c->ev_ex, *mom = c->ev_psi;
+    PCE_CUDA(c, cudaMemsetAsync(zeros, 0, (size_t)N * sizeof(double), c->st));
+    std::vector<double> h((size_t)4 * nb);
+    for (int d = 0; d < 3; ++d) {
+        const double E0[3] = {d == 0 ? 1.0 : 0.0, d == 1 ? 1.0 : 0.0, d == 2 ? 1.0 : 0.0};
+        pce_solve_info inf;
+        int rc = solve_cg(c, zeros, zeros, E0, 0, q, Phi, &inf);
+        if (rc != PCE_OK && rc != PCE_ENOCONV) return rc;
+        if (rc == PCE_ENOCONV) rc_all = PCE_ENOCONV;
+        k_cap_moments<<<nb, BT, 0, c->st>>>(nb, c->body_off, q, c->rx, c->ry, c->rz, mom);
+        c->launches++;
+        PCE_CUDA(c, cudaMemcpyAsync(h.data(), mom, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+        PCE_CUDA(c, cudaStreamSynchronize(c->st));
+        for (int e = 0; e < 3; ++e) {
+            double s = 0.0;
+            for (int i = 0; i < nb; ++i) s += h[(size_t)nb + 3 * i + e];
+            eps_eff[3 * e + d] = (e == d ? c->p.eps_f : 0.0) + s / c->V;
+        }
+        worst.iters = worst.iters > inf.iters ? worst.iters : inf.iters;
+        worst.matvecs += inf.matvecs;
+        worst.rel_resid = worst.rel_resid > inf.rel_resid ? worst.rel_resid : inf.rel_resid;
+        worst.converged = worst.converged && inf.converged;
+    }
+    if (info) *info = worst;
+    return rc_all;
+}

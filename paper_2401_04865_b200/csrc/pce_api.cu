@@ -506,6 +506,30 @@ extern "C" int pce_forces(pce_ctx* c, const double* q, const double E0[3], doubl
     return rc;
 }
 
+extern "C" int pce_capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_solve_info* info)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_capacitance_columns before pce_set_system"; return PCE_ESTATE; }
+    if (ncol < 0 || (ncol > 0 && (!cols || !C))) { c->err = "NULL argument"; return PCE_EINVAL; }
+    if (c->Nbody == 0 || c->Nbead == 0) { c->err = "pce_capacitance_columns: the system has no conductor bodies"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = capacitance_columns(c, ncol, cols, C, info);
+    timing_end(c);
+    return rc;
+}
+
+extern "C" int pce_effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_effective_permittivity before pce_set_system"; return PCE_ESTATE; }
+    if (!eps_eff) { c->err = "NULL argument"; return PCE_EINVAL; }
+    if (c->Nbody == 0 || c->Nbead == 0) { c->err = "pce_effective_permittivity: the system has no conductor bodies"; return PCE_EINVAL; }
+    timing_begin(c);
+    int rc = effective_permittivity(c, eps_eff, info);
+    timing_end(c);
+    return rc;
+}
+
 // ---------------------------------------------------------------- host-buffer pass (bench "e2e")
 extern "C" int pce_step_host(pce_ctx* c, const double* x, const double* y, const double* z, const double* Q_body, const double* q_ion,
                              const double E0[3], double* q, double* Phi_body, double* fx, double* fy, double* fz, double* F, double* T,

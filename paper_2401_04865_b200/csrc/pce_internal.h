@@ -286,6 +286,8 @@ int wave_gather_cols(pce_ctx* c, const Bins& b, bool field, double* psi_s, doubl
 int bodies_setup(pce_ctx* c);
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
 int solve_plain(pce_ctx* c, const double* b, double* q, pce_solve_info* info);  // M_bb q = b (no constraint), b and q device [Nbead]
+int capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_solve_info* info);
+int effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info);
 void krylov_free(pce_ctx* c);
 void krylov_invalidate_graph(pce_ctx* c);
 int op_matvec_bead_sorted(pce_ctx* c);  // sorted charges in bead.qs / wbead.qs -> w_real / w_wave (sorted orders)

@@ -35,6 +35,14 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+// the same, issued only if `on` != 0 (warp-uniform): a predicated DMMA, no branch and no re-convergence code around it
+__device__ __forceinline__ void dmma884_if(unsigned on, double& d0, double& d1, double a, double b)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+                 "@p mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n\t}"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b), "r"(on));
+}
+
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -201,7 +209,7 @@ template <int STRIDE>
 struct alignas(16) WarpSmem {
     double wt[32 * STRIDE];                 // brick-local weights of the current batch
     unsigned char rec[32 * REC_BYTES];      // hit records of the batch being loaded (16-byte chunks XOR-swizzled by hit index)
-    unsigned char mask[40];                 // live planes of each hit of the current batch (0 beyond the batch)
+    unsigned char mask[16];                 // live planes of each mma group of the current batch
 };
 
 struct Item {
@@ -277,24 +285,26 @@ template <bool FIELD>
 __device__ __forceinline__ unsigned brick_weights(int P, const double* __restrict__ tab, int b0, int ng, int s0, const double4 cf, double u0,
                                                   double scale, double* __restrict__ w)
 {
-    const int dsl = wrap_once(b0 - s0, ng);
-    const int r0 = (dsl < P) ? dsl : dsl - ng;   // support index of brick-local point 0: -7 .. P-1
+    int r0 = b0 - s0;                   // support index of brick-local point 0, brought into -7 .. P-1
+    if (r0 >= P) r0 -= ng;
+    if (r0 < -7) r0 += ng;
     const int phi = (-s0) & (BR - 1);
-    const int m = (r0 - phi) >> 3;               // -1 .. 3
-    const double e82 = cf.z * cf.z;
-    const double pm = (m < 0) ? cf.w : (m == 0) ? 1.0 : (m == 1) ? cf.z : (m == 2) ? e82 : e82 * cf.z;
+    const int m = (r0 - phi) >> 3;      // -1 .. 3: r0 = phi + 8 m
+    double pm = (m < 0) ? cf.w : 1.0;   // e8^m
+    if (m >= 1) pm = cf.z;
+    if (m >= 2) pm *= cf.z;
+    if (m >= 3) pm *= cf.z;
     double pw = cf.x * pm * tab[r0 + 8] * scale;
     double t = cf.y * tab[48 + r0 + 8];
-    const double g2 = tab[9] * tab[9];           // exp(-2 aw)
+    const double g2 = tab[9] * tab[9];  // exp(-2 aw)
+    // live points j: 0 <= r0 + j < P
+    const int lo = max(0, -r0), hi = min(BR, P - r0);
+    const unsigned live = ((1u << hi) - 1u) & ~((1u << lo) - 1u);
     double v[BR], vu[BR];
-    unsigned live = 0;
 #pragma unroll
     for (int j = 0; j < BR; ++j) {
-        const int r = r0 + j;
-        const bool in = (unsigned)r < (unsigned)P;
-        v[j] = in ? pw : 0.0;
-        live |= (in ? 1u : 0u) << j;
-        if (FIELD) vu[j] = v[j] * (u0 + (double)r);
+        v[j] = (live & (1u << j)) ? pw : 0.0;
+        if (FIELD) vu[j] = v[j] * (u0 + (double)(r0 + j));
         pw *= t;
         t *= g2;
     }
@@ -317,7 +327,7 @@ __device__ __forceinline__ void load_tables(const WaveConst& wc, double* tab)
 }
 
 // weights of the nh hits whose records sit in the warp's buffer (one hit per lane): table rows + live-plane masks
-template <bool FIELD, int STRIDE, int DW>
+template <bool FIELD, int STRIDE, int DW, int GROUP>
 __device__ __forceinline__ void batch_weights(const WaveConst& wc, const double* __restrict__ tab, const Item& it, WarpSmem<STRIDE>& s, int nh,
                                               int lane, bool use_q, double4 u0v)
 {
@@ -336,8 +346,11 @@ __device__ __forceinline__ void batch_weights(const WaveConst& wc, const double*
             if (d == 2) zmask = lv;
         }
     }
-    s.mask[lane] = (unsigned char)zmask;
-    if (lane < 8) s.mask[32 + lane] = 0;
+    // planes live for any hit of an mma group (GROUP = 4 hits in the spread, 8 in the gather): one byte per group
+    zmask |= __shfl_xor_sync(0xffffffffu, zmask, 1);
+    zmask |= __shfl_xor_sync(0xffffffffu, zmask, 2);
+    if (GROUP == 8) zmask |= __shfl_xor_sync(0xffffffffu, zmask, 4);
+    if ((lane & (GROUP - 1)) == 0) s.mask[lane / GROUP] = (unsigned char)zmask;
     __syncwarp();
 }
 
@@ -373,7 +386,7 @@ k_spread_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
             const int nh = min(32, it.h1 - hb);
             cp_async_wait_all();
             __syncwarp();
-            batch_weights<false, STRIDE_PSI, BR>(wc, tab, it, s, nh, lane, true, make_double4(0, 0, 0, 0));
+            batch_weights<false, STRIDE_PSI, BR, 4>(wc, tab, it, s, nh, lane, true, make_double4(0, 0, 0, 0));
             if (hb + 32 < it.h1) {  // the records are consumed: start the next batch's
                 prefetch_records(s.rec, rec, p_next, lane);
                 p_next = hit_slot(it, ent, hb + 64 + lane);
@@ -383,14 +396,20 @@ k_spread_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                 const double* w = s.wt + (live ? sb + t : 0) * STRIDE_PSI;
                 const double bx = live ? w[gq] : 0.0;        // B[t][gq] = wx_h[x = gq]
                 const double ay = live ? w[BR + gq] : 0.0;   // wy_h[y = gq]
-                const unsigned m4 = *reinterpret_cast<const unsigned*>(s.mask + sb);
-                const unsigned m = (m4 | (m4 >> 8) | (m4 >> 16) | (m4 >> 24)) & 0xffu;  // planes live for any hit of the group
+                const unsigned m = s.mask[sb >> 2];          // planes live for any hit of the group
+                if (m == 0xffu) {  // the common case: every plane live
 #pragma unroll
-                for (int z = 0; z < BR; z += 2) {
-                    if (m & (3u << z)) {
+                    for (int z = 0; z < BR; z += 2) {
                         const double2 wz = *reinterpret_cast<const double2*>(w + 2 * BR + z);  // q_h wz_h[z], [z + 1]
-                        if (m & (1u << z)) dmma884(acc[z][0], acc[z][1], ay * wz.x, bx);
-                        if (m & (2u << z)) dmma884(acc[z + 1][0], acc[z + 1][1], ay * wz.y, bx);
+                        dmma884(acc[z][0], acc[z][1], ay * wz.x, bx);
+                        dmma884(acc[z + 1][0], acc[z + 1][1], ay * wz.y, bx);
+                    }
+                } else {
+#pragma unroll
+                    for (int z = 0; z < BR; z += 2) {
+                        const double2 wz = *reinterpret_cast<const double2*>(w + 2 * BR + z);
+                        dmma884_if(m & (1u << z), acc[z][0], acc[z][1], ay * wz.x, bx);
+                        dmma884_if(m & (2u << z), acc[z + 1][0], acc[z + 1][1], ay * wz.y, bx);
                     }
                 }
             }
@@ -478,7 +497,7 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
             const int nh = min(32, it.h1 - hb);
             cp_async_wait_all();
             __syncwarp();
-            batch_weights<FIELD, STRIDE, DW>(wc, tab, it, s, nh, lane, false, u_cur);
+            batch_weights<FIELD, STRIDE, DW, 8>(wc, tab, it, s, nh, lane, false, u_cur);
             const int p_mine = p_cur;  // slot of hit hb + lane (output index)
             p_cur = p_next; u_cur = u_next;
             if (hb + 32 < it.h1) {
@@ -492,28 +511,33 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                 const double* w = s.wt + (live ? hr : 0) * STRIDE;
                 const double a0 = live ? w[DW + t] : 0.0, a1 = live ? w[DW + t + 4] : 0.0;  // wy_h[y]
                 const double2 wx2 = *reinterpret_cast<const double2*>(w + 2 * t);           // wx_h[2t], [2t + 1]
-                const uint2 m8 = *reinterpret_cast<const uint2*>(s.mask + sb);
-                unsigned m = m8.x | m8.y;
-                m = (m | (m >> 8) | (m >> 16) | (m >> 24)) & 0xffu;
+                const unsigned m = s.mask[sb >> 3];  // planes live for any hit of the group
                 const int po = __shfl_sync(0xffffffffu, p_mine, hr & 31);
                 if (!FIELD) {
                     double u0 = 0.0, u1 = 0.0;
+                    if (m == 0xffu) {  // the common case: every plane live
 #pragma unroll
-                    for (int z = 0; z < BR; z += 2) {
-                        if (m & (3u << z)) {
+                        for (int z = 0; z < BR; z += 2) {
                             const double2 wz = *reinterpret_cast<const double2*>(w + 2 * DW + z);
-                            if (m & (1u << z)) {
-                                double t0 = 0.0, t1 = 0.0;
-                                dmma884(t0, t1, a0, H[z][0]);
-                                dmma884(t0, t1, a1, H[z][1]);
-                                u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);
-                            }
-                            if (m & (2u << z)) {
-                                double t0 = 0.0, t1 = 0.0;
-                                dmma884(t0, t1, a0, H[z + 1][0]);
-                                dmma884(t0, t1, a1, H[z + 1][1]);
-                                u0 = fma(wz.y, t0, u0); u1 = fma(wz.y, t1, u1);
-                            }
+                            double t0 = 0.0, t1 = 0.0, s0 = 0.0, s1 = 0.0;
+                            dmma884(t0, t1, a0, H[z][0]);
+                            dmma884(t0, t1, a1, H[z][1]);
+                            dmma884(s0, s1, a0, H[z + 1][0]);
+                            dmma884(s0, s1, a1, H[z + 1][1]);
+                            u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);
+                            u0 = fma(wz.y, s0, u0); u1 = fma(wz.y, s1, u1);
+                        }
+                    } else {
+#pragma unroll
+                        for (int z = 0; z < BR; z += 2) {
+                            const double2 wz = *reinterpret_cast<const double2*>(w + 2 * DW + z);
+                            double t0 = 0.0, t1 = 0.0, s0 = 0.0, s1 = 0.0;  // dead planes: the products stay 0
+                            dmma884_if(m & (1u << z), t0, t1, a0, H[z][0]);
+                            dmma884_if(m & (1u << z), t0, t1, a1, H[z][1]);
+                            dmma884_if(m & (2u << z), s0, s1, a0, H[z + 1][0]);
+                            dmma884_if(m & (2u << z), s0, s1, a1, H[z + 1][1]);
+                            u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);
+                            u0 = fma(wz.y, s0, u0); u1 = fma(wz.y, s1, u1);
                         }
                     }
                     double r = fma(wx2.y, u1, wx2.x * u0);
@@ -526,17 +550,16 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                     double u0 = 0.0, u1 = 0.0, uz0 = 0.0, uz1 = 0.0, uy0 = 0.0, uy1 = 0.0;
 #pragma unroll
                     for (int z = 0; z < BR; ++z) {
-                        if (m & (1u << z)) {
-                            const double wz = w[2 * DW + z], wzu = w[2 * DW + BR + z];
-                            double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;
-                            dmma884(t0, t1, a0, H[z][0]);
-                            dmma884(t0, t1, a1, H[z][1]);
-                            dmma884(v0, v1, b0, H[z][0]);
-                            dmma884(v0, v1, b1, H[z][1]);
-                            u0 = fma(wz, t0, u0); u1 = fma(wz, t1, u1);
-                            uz0 = fma(wzu, t0, uz0); uz1 = fma(wzu, t1, uz1);
-                            uy0 = fma(wz, v0, uy0); uy1 = fma(wz, v1, uy1);
-                        }
+                        const double wz = w[2 * DW + z], wzu = w[2 * DW + BR + z];
+                        double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;
+                        const unsigned on = m & (1u << z);
+                        dmma884_if(on, t0, t1, a0, H[z][0]);
+                        dmma884_if(on, t0, t1, a1, H[z][1]);
+                        dmma884_if(on, v0, v1, b0, H[z][0]);
+                        dmma884_if(on, v0, v1, b1, H[z][1]);
+                        u0 = fma(wz, t0, u0); u1 = fma(wz, t1, u1);
+                        uz0 = fma(wzu, t0, uz0); uz1 = fma(wzu, t1, uz1);
+                        uy0 = fma(wz, v0, uy0); uy1 = fma(wz, v1, uy1);
                     }
                     double r0 = fma(wx2.y, u1, wx2.x * u0);      // psi
                     double r1 = fma(wxu2.y, u1, wxu2.x * u0);    // sum W u_x H

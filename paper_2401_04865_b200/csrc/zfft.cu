@@ -136,6 +136,10 @@ __device__ __forceinline__ double shape_eval(const double* __restrict__ tab, int
     return ((c67.y * t + c67.x) * t2 + (c45.y * t + c45.x)) * t4 + ((c23.y * t + c23.x) * t2 + (c01.y * t + c01.x));
 }
 
+// last forward stage x Green's function x first inverse stage on the tile column sp (stride KP), in place
+template <int N, int R>
+__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs);
+
 template <int N> struct Radices {
     static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;  // N = 8^m * rest
     static constexpr int n8 = (N == 16 || N == 32 || N == 64) ? (N == 64 ? 2 : 1) : (N == 128 || N == 256 || N == 512) ? (N == 512 ? 3 : 2) : 3;
@@ -144,6 +148,32 @@ template <int N> struct Radices {
 // forward (S = -1): stages 8 (global -> smem), 8.., rest (-> smem);  inverse (S = +1): 8 (smem, scaled -> smem), 8.., rest (-> global)
 // KP pencils per CTA, N/8 threads per pencil.  zexp = [ex | ey | ez]: exp(-gexp_d k_d^2) per axis (host tables).
 constexpr int KP = 4;
+template <int N, int R>
+__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs)
+{
+    constexpr int NB = 8 / R, NTH = N / 8;
+    double2 v[8];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int b = j + q * NTH;
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[q * R + r] = sp[(size_t)(b + r * (N / R)) * KP];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int b = j + q * NTH;  // b < N / R = Ns: k = b, twiddle step k N / (Ns R) = b
+        twiddle_dft<R, -1>(v + q * R, b, tw);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double gf = gs[(b + r * (N / R)) * KP + p];
+            v[q * R + r].x *= gf; v[q * R + r].y *= gf;
+        }
+        dftR<R, +1>(v + q * R);  // Ns = 1: no twiddles; outputs at b R + r
+#pragma unroll
+        for (int r = 0; r < R; ++r) sp[(size_t)(b * R + r) * KP] = v[q * R + r];
+    }
+}
 template <int N>
 __global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
 k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
@@ -180,38 +210,30 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
         }
     }
     const int my = (iy == 0 || 2 * iy == ny) ? -1 : ny - iy;  // mirror row: same |k_y|
+    constexpr int NF8 = (REST == 8) ? N8 - 1 : N8;  // radix-8 stages before the fused one
     for (int pass = 0; pass < 2; ++pass) {
         const int y = pass == 0 ? iy : my;
         if (y < 0) break;
         double2* col = gk + (size_t)y * nxh + (col_ok ? kxi : 0);
         double2* sp = tile + p;
         __syncthreads();  // twiddles and Green's function stored / previous pass done with the tile
-        double g[8];
-#pragma unroll
-        for (int r = 0; r < 8; ++r) g[r] = gs[(j + r * (N / 8)) * KP + p];
-        // ---- forward
+        // ---- forward: the first stage reads global memory; all but the last stage of the transform here
         stage<N, 8, -1, false>(col, zstr, col_ok, sp, KP, true, 1, j, tw, nullptr);
         __syncthreads();
         int Ns = 8;
-        if (N8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        if (N8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        if (REST != 8) { stage<N, REST, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); }
-        // ---- scale + inverse
-        if (REST != 8 || N8 > 1) {
-            stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, 1, j, tw, g);
-            __syncthreads();
-            Ns = 8;
-            if (N8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-            if (REST != 8) {
-                if (N8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-                stage<N, REST, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
-            } else {
-                stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
-            }
-        }
+        if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        // ---- last forward stage (radix REST, Ns = N / REST) x Green's function x first inverse stage (radix REST, Ns = 1), in
+        // registers: the forward stage leaves element b + r N/REST in slot r, which is what the inverse stage reads
+        fused_middle<N, REST>(sp, j, p, tw, gs);
+        __syncthreads();
+        // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
+        Ns = REST;
+        if (NF8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        if (NF8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
     }
 }
-
 
 // ---------------------------------------------------------------- pipelined variant (N_z = 64 ... 1024 with N = 8^m * rest)
 // Same arithmetic, arranged so that HBM is kept busy: persistent CTAs walk (k_x tile, |k_y|) pairs; the [N_z][KP] tile of the
@@ -306,32 +328,9 @@ k_zfft_scale_pipe(WaveConst wc, double2* __restrict__ gk, const double2* __restr
         if (NF8 >= 1) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        // ---- last forward stage (radix REST, Ns = N / REST) x Green's function x first inverse stage (radix REST, Ns = 1)
-        {
-            constexpr int R = REST, NB = 8 / R, NTH = N / 8;
-            double2 v[8];
-#pragma unroll
-            for (int q = 0; q < NB; ++q) {
-                const int b = j + q * NTH;
-#pragma unroll
-                for (int r = 0; r < R; ++r) v[q * R + r] = sp[(size_t)(b + r * (N / R)) * KP];
-            }
-            __syncthreads();
-#pragma unroll
-            for (int q = 0; q < NB; ++q) {
-                const int b = j + q * NTH;  // b < N / R = Ns: k = b, twiddle step k N / (Ns R) = b
-                twiddle_dft<R, -1>(v + q * R, b, tw);
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const double gf = gs[(b + r * (N / R)) * KP + p];
-                    v[q * R + r].x *= gf; v[q * R + r].y *= gf;
-                }
-                dftR<R, +1>(v + q * R);  // Ns = 1: no twiddles; outputs at b R + r
-#pragma unroll
-                for (int r = 0; r < R; ++r) sp[(size_t)(b * R + r) * KP] = v[q * R + r];
-            }
-            __syncthreads();
-        }
+        // ---- last forward stage x Green's function x first inverse stage, in registers
+        fused_middle<N, REST>(sp, j, p, tw, gs);
+        __syncthreads();
         // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
         Ns = REST;
         if (NF8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
@@ -424,8 +423,8 @@ int zfft_init(pce_ctx* c)
 
 int zfft_scale(pce_ctx* c)
 {
-    static const bool no_pipe = [] { const char* e = getenv("PCE_ZFFT_PIPE"); return e && e[0] == '0'; }();
-    if (!no_pipe) {  // pipelined variant: meshes with at least two radix stages
+    static const bool pipe = [] { const char* e = getenv("PCE_ZFFT_PIPE"); return e && e[0] == '1'; }();
+    if (pipe) {  // pipelined variant (persistent CTAs, cp.async double buffer): measured slower on B200 (fewer resident warps), kept for experiments
         switch (c->p.Ng[2]) {
             case 64: return launch_pipe<64>(c);
             case 128: return launch_pipe<128>(c);

@@ -414,3 +414,59 @@ def test_dR_small_r_branch():
         lim = -1.0 / (16 * np.pi * a * a)
         for r in (1e-9 * a, 0.5e-6 * a, 0.99e-6 * a, 1.01e-6 * a, 2e-6 * a, 1e-5 * a):
             assert orc.dR(r, a, xi) == pytest.approx(lim, rel=2e-4), (a, xi, r)
+
+
+# ---------------------------------------------------------------- grand capacitance tensor (eq. 15) and eps_eff (eq. 36-37)
+def test_capacitance_tensor_symmetry_and_cubic_cell_couplings():
+    """C = Sigma' M^-1 Sigma'^T is symmetric positive definite; for one sphere in a cubic periodic cell the couplings
+    C_qE and C_SPsi vanish by symmetry and C_SE = (S / E0) I with S the dipole of the constrained solve of
+    eq. 13 (an independent route: dense KKT system instead of M^-1)."""
+    w = wl.config1(subdiv=1, L=6.0)
+    C = orc.capacitance(w.x, w.body_offset, w.L, w.a)
+    assert C.shape == (4, 4)
+    assert np.abs(C - C.T).max() < 1e-12 * np.abs(C).max()
+    assert np.linalg.eigvalsh(0.5 * (C + C.T)).min() > 0
+    assert np.abs(C[0, 1:]).max() < 1e-11 and np.abs(C[1:, 0]).max() < 1e-11
+    q, Phi, _ = orc.solve_induced(w.x, w.body_offset, [0.0], [], [0, 0, 1.0], w.L, w.a)
+    S = (orc.rel_positions(w.x, w.body_offset, w.L) * q[:, None]).sum(0)
+    assert np.abs(C[1:, 1:] - S[2] * np.eye(3)).max() < 1e-10 * S[2]
+    eps = orc.effective_permittivity(C, 1, float(np.prod(w.L)))
+    assert np.abs(eps - (1 + S[2] / np.prod(w.L)) * np.eye(3)).max() < 1e-12
+
+
+def test_capacitance_of_a_sphere_in_a_periodic_cell_textbook_value():
+    """C_qPsi of one conducting sphere of radius R in a cubic cell with neutralising background (k = 0 removed,
+    PAPER.md:80): Psi/Q = 1/(4 pi R) - zeta/(4 pi L) + R^2/(6 V) + ..., zeta = 2.837297 the textbook Madelung constant
+    of a simple-cubic lattice of point charges in a uniform background.  The bead model makes R an effective radius
+    a little above 1: checked to 3 %."""
+    w = wl.config1(subdiv=3, L=10.0)
+    C = orc.capacitance(w.x, w.body_offset, w.L, w.a)
+    L = 10.0
+    inv_exact = 1 / (4 * np.pi) - 2.837297 / (4 * np.pi * L) + 1.0 / (6 * L ** 3)
+    assert 1 / C[0, 0] == pytest.approx(inv_exact, rel=0.03)
+    assert 1 / C[0, 0] < inv_exact  # a_eff > R: slightly larger capacitance
+
+
+def test_effective_permittivity_matches_the_constrained_solves_and_dilute_limit():
+    """eq. 36 from the blocks of C (Schur complement C_SE - C_SPsi C_qPsi^-1 C_qE) must equal the mean dipole of the
+    constrained solves of eq. 13 with Q = 0 and unit fields, for bodies with no symmetry; and for a dilute cubic array it
+    approaches the Clausius-Mossotti value 1 + 3 phi_eff / (1 - phi_eff)."""
+    w = wl.tiny_random(seed=41, n_body=3, n_ion=0, L=7.0, a=0.2)
+    nb, V = w.N_body, float(np.prod(w.L))
+    C = orc.capacitance(w.x, w.body_offset, w.L, w.a)
+    eps = orc.effective_permittivity(C, nb, V)
+    ref = np.eye(3)
+    for d in range(3):
+        E0 = np.eye(3)[d]
+        q, Phi, _ = orc.solve_induced(w.x, w.body_offset, np.zeros(nb), [], E0, w.L, w.a)
+        o = orc.forces_torques(w.x, w.body_offset, q, E0, w.L, w.a, Phi_body=Phi)
+        ref[:, d] += o["S"].sum(0) / V
+    assert np.abs(eps - ref).max() < 1e-10
+    assert np.abs(eps - eps.T).max() < 1e-10
+    # dilute simple-cubic array of spheres (one per cell)
+    w1 = wl.config1(subdiv=2, L=8.0)
+    C1 = orc.capacitance(w1.x, w1.body_offset, w1.L, w1.a)
+    e1 = orc.effective_permittivity(C1, 1, 8.0 ** 3)
+    phi_eff = (e1[2, 2] - 1) / (e1[2, 2] + 2)  # invert Clausius-Mossotti: phi = (eps - 1)/(eps + 2)
+    phi_geo = 4 * np.pi / 3 / 8.0 ** 3
+    assert 1.0 < phi_eff / phi_geo < 1.25  # effective radius a few per cent above the geometric one (PAPER.md:280)
