@@ -9,3 +9,4 @@ from .oracle import (  # noqa: F401
     build, M_free, R, R0, dR, ewald_eval, pair_matrix, body_centres, rel_positions,
     solve_induced, forces_torques, default_xi, num_threads, sigma_prime, capacitance, effective_permittivity,
 )
+from . import dynamics  # noqa: F401,E402  (Brownian-dynamics step and double-layer observables)
