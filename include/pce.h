@@ -192,6 +192,43 @@ int pce_capacitance_columns(pce_ctx* ctx, int ncol, const int* cols, double* C, 
  * columns); the oracle evaluates eq. 36 from the blocks of C literally.  eps_eff: host [9], row-major. */
 int pce_effective_permittivity(pce_ctx* ctx, double eps_eff[9], pce_solve_info* info);
 
+/* Parameters of one Brownian-dynamics step. */
+typedef struct {
+    double dt;              /* time step (eq. 44) */
+    double gamma;           /* Stokes drag coefficient of every ion and bead (eq. 43) */
+    double kT;              /* thermal energy (eq. 41) */
+    unsigned long long seed; /* key of the counter-based generator (used when `noise` is NULL) */
+    unsigned int step;      /* time-step index: second counter word of the generator */
+    int move_bodies;        /* 0: conductor bodies held fixed; 1: free-draining rigid-body motion (eq. 62) */
+} pce_bd_params;
+
+/* One Euler-Maruyama step of the overdamped Langevin equation (eqs. 40-44) from the context's current
+ * positions, all on the device:
+ *   hard spheres: eq. 46 as a pair potential at x(t): particles of different bodies closer than 2a repel
+ *     with |f| = gamma (2a - r) / (2 dt), i.e. one step puts an overlapping pair back in contact; linked cells
+ *     of edge >= 2a;
+ *   ions: x += (f + f_hs) dt / gamma + sqrt(2 kT dt / gamma) N(0,1)  (eqs. 41-44).  N(0,1): `noise` (device, 3 N_ion doubles
+ *     as x[N_ion], y[N_ion], z[N_ion]) or, if NULL, Philox-4x32-10 (counter = (ion index, step, 0, 0), key = seed) with
+ *     Box-Muller on (r + 1/2) 2^-32: (sqrt(-2 ln u0) cos 2 pi u1, sqrt(-2 ln u0) sin 2 pi u1, sqrt(-2 ln u2) cos 2 pi u3);
+ *   bodies (move_bodies): F_i, L_i of eq. 18 from f + f_hs, free-draining mobility (no hydrodynamic interactions,
+ *     PAPER.md:382): U = F / (N_i gamma), Omega = [gamma sum_j (r_j^2 I - r_j r_j^T)]^-1 L, X += U dt, r_ij turned by the
+ *     rotation exp([Omega dt]_x) (eq. 62 with U, Omega constant over the step); no Brownian displacement of bodies.
+ * fx, fy, fz: device [N], the electrostatic forces of pce_forces (eq. 17).  The context then advances to the new positions
+ * exactly as by pce_set_positions; x, y, z (device [N], may be NULL) receive them (wrapped into the box, caller order). */
+int pce_bd_step(pce_ctx* ctx, const pce_bd_params* bp, const double* fx, const double* fy, const double* fz,
+                const double* noise, double* x, double* y, double* z);
+
+/* Double-layer observables about the centre of conductor body `body` from the context's current
+ * positions and the charges q (device [N]): shells k = 0..n_bins-1 = [r_lo + k dr, r_lo + (k+1) dr), dr = 0.1 a
+ * (PAPER.md:419), minimum-image distances of the IONS from the body centre.
+ *   counts : device [2 n_bins]: cations (q > 0) then anions (q < 0) per shell ("shell summation")
+ *   g      : device [2 n_bins]: eq. 49, count / (n_species * shell volume), n_species = N_species / V
+ *   rho    : device [n_bins]: radial charge density, sliding window of width 2a about the shell midpoint
+ *   Qcum   : device [n_bins]: eq. 48, Q + sum_{j<=k} rho_j dr, Q = net charge of the body's beads
+ * Any output may be NULL. */
+int pce_radial_profile(pce_ctx* ctx, int body, const double* q, double r_lo, int n_bins,
+                       double* counts, double* g, double* rho, double* Qcum);
+
 /* One whole pass of the hot path from HOST buffers (what bench.py's "e2e"
  * times): copy positions and charges to the device, rebuild cells, solve
  * eq. 13, evaluate forces, copy results back.  All pointers host; x,y,z [N];

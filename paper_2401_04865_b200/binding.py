@@ -22,7 +22,7 @@ EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
     "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks", "pce_debug_poison_shared_memory",
-    "pce_capacitance_columns", "pce_effective_permittivity",
+    "pce_capacitance_columns", "pce_effective_permittivity", "pce_bd_step", "pce_radial_profile",
 )
 
 
@@ -34,6 +34,11 @@ class PceParams(C.Structure):
 
 class PceSolveInfo(C.Structure):
     _fields_ = [("iters", C.c_int), ("matvecs", C.c_int), ("rel_resid", C.c_double), ("converged", C.c_int)]
+
+
+class PceBdParams(C.Structure):
+    _fields_ = [("dt", C.c_double), ("gamma", C.c_double), ("kT", C.c_double), ("seed", C.c_ulonglong), ("step", C.c_uint),
+                ("move_bodies", C.c_int)]
 
 
 class PceTimings(C.Structure):
@@ -92,6 +97,8 @@ def load():
     lib.pce_debug_poison_shared_memory.argtypes = [vp]
     lib.pce_capacitance_columns.argtypes = [vp, C.c_int, ip, vp, C.POINTER(PceSolveInfo)]
     lib.pce_effective_permittivity.argtypes = [vp, dp, C.POINTER(PceSolveInfo)]
+    lib.pce_bd_step.argtypes = [vp, C.POINTER(PceBdParams)] + [vp] * 7
+    lib.pce_radial_profile.argtypes = [vp, C.c_int, vp, C.c_double, C.c_int] + [vp] * 4
     lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
@@ -263,6 +270,28 @@ class Context:
         self._ck(self.lib.pce_effective_permittivity(self.h, out, C.byref(info)))
         return np.array(list(out)).reshape(3, 3), {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid,
                                                     "converged": bool(info.converged)}
+
+    def bd_step(self, f, dt, gamma=1.0, kT=1.0, seed=0, step=0, move_bodies=False, noise=None):
+        """One Brownian-dynamics step (eqs. 40-46, 62) from the context's positions; f: (N, 3) forces of forces().
+        noise: optional (N_ion, 3) standard normals (else the library's Philox stream).  Returns the new x, y, z."""
+        fx, fy, fz = (f[:, d].contiguous() for d in range(3))
+        for t in (fx, fy, fz):
+            self._chk(t, self.N)
+        nz = None
+        if noise is not None:
+            nz = noise.T.contiguous().view(-1)
+            self._chk(nz, 3 * (self.N - self.N_bead))
+        bp = PceBdParams(float(dt), float(gamma), float(kT), int(seed), int(step), int(bool(move_bodies)))
+        x, y, z = self._new(self.N), self._new(self.N), self._new(self.N)
+        self._ck(self.lib.pce_bd_step(self.h, C.byref(bp), _ptr(fx), _ptr(fy), _ptr(fz), _ptr(nz), _ptr(x), _ptr(y), _ptr(z)))
+        return x, y, z
+
+    def radial_profile(self, body, q, r_lo, n_bins):
+        """Shell counts, g(r) (eq. 49), windowed charge density and Q'(r) (eq. 48) of the ions about a body's centre."""
+        self._chk(q, self.N)
+        counts, g, rho, Qc = self._new(2 * n_bins), self._new(2 * n_bins), self._new(n_bins), self._new(n_bins)
+        self._ck(self.lib.pce_radial_profile(self.h, int(body), _ptr(q), float(r_lo), int(n_bins), _ptr(counts), _ptr(g), _ptr(rho), _ptr(Qc)))
+        return {"counts": counts.view(2, n_bins).T, "g": g.view(2, n_bins).T, "rho": rho, "Qcum": Qc}
 
     def step_host(self, x, y, z, Q_body, q_ion, E0, out):
         """Host-buffer pass.  x,y,z,Q_body,q_ion: host numpy/pinned-torch f64; ``out``: dict of host arrays

@@ -77,6 +77,7 @@ static void free_system(pce_ctx* c)
     krylov_invalidate_graph(c);
     cudaFree(c->hs_dev); cudaFree(c->cg_z); cudaFree(c->pc_mean);
     precond_free(c);
+    dynamics_free(c);
     c->cg_z = c->pc_mean = nullptr;
     c->x = c->y = c->z = nullptr; c->body_off = c->body_of = nullptr;
     c->rx = c->ry = c->rz = c->X = c->Y = c->Z = nullptr;
@@ -255,6 +256,8 @@ static int positions_impl(pce_ctx* c, const double* x, const double* y, const do
     if ((rc = real_csr_build(c, c->bead))) return rc;
     return PCE_OK;
 }
+
+int positions_update(pce_ctx* c, const double* x, const double* y, const double* z) { return positions_impl(c, x, y, z); }
 
 extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_offset, const double* x, const double* y, const double* z)
 {

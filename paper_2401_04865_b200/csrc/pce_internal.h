@@ -185,6 +185,13 @@ struct pce_ctx {
     double* pc_mean = nullptr;        // [Nbody]
     double* pc_u = nullptr;           // [Nbead] u = A^-1 1 of each body's block (0: no block)
     double* pc_invs = nullptr;        // [Nbody] 1 / (1.u)
+    // Brownian dynamics (dynamics.cu): linked cells of edge >= 2a, hard-sphere forces, the new positions, profile counters
+    Bins hs;
+    bool hs_ready = false;
+    double *bd_f = nullptr;   // [3 N] hard-sphere forces, caller order (x | y | z)
+    double *bd_x = nullptr;   // [3 N] new positions (x | y | z)
+    unsigned* prof_cnt = nullptr;  // [2 n_bins] shell counts
+    int prof_cnt_n = 0;
     // host staging for pce_step_host
     double* hs_dev = nullptr;
     size_t hs_dev_n = 0;
@@ -293,6 +300,10 @@ void krylov_invalidate_graph(pce_ctx* c);
 int op_matvec_bead_sorted(pce_ctx* c);  // sorted charges in bead.qs / wbead.qs -> w_real / w_wave (sorted orders)
 int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
                double* S, double* U_body, double* U_tot, double* psi_out);
+
+// dynamics.cu
+void dynamics_free(pce_ctx* c);
+int positions_update(pce_ctx* c, const double* x, const double* y, const double* z);  // pce_api.cu: what pce_set_positions does
 
 // precond.cu
 int precond_setup(pce_ctx* c);

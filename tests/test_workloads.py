@@ -64,24 +64,3 @@ def test_config5_replica_self_checks():
     t = geo.fibonacci_spheroid(1000)
     d, _ = cKDTree(t).query(t, k=2)
     assert d[:, 1].max() / d[:, 1].min() < 1.6
-
-
-def test_bd_harness_keeps_hard_sphere_constraints():
-    """workloads/dynamics.py (eqs. 42-46): after a step no two ions overlap, none sits inside the colloid's
-    excluded shell, all are wrapped; zero force and zero noise leave a valid configuration unchanged."""
-    import numpy as np
-    from scipy.spatial import cKDTree
-    import workloads as wl
-    w = wl.config3(n_salt=500)
-    L, a, c = float(w.L[0]), w.a, np.full(3, w.L[0] / 2)
-    x0 = w.x[w.N_bead:].copy()
-    same = wl.dynamics.bd_step(x0.copy(), np.zeros_like(x0), np.zeros_like(x0), 1e-7, L, a, c, 1.0)
-    assert np.allclose(same, x0, atol=1e-14)
-    noise = wl.dynamics.noise_for(11, 1, w.N_ion)[0]
-    x1 = wl.dynamics.bd_step(x0.copy(), np.ones_like(x0), noise, 2e-3, L, a, c, 1.0, sweeps=50)  # large step: many overlaps
-    assert x1.min() >= 0 and x1.max() < L
-    assert len(cKDTree(x1, boxsize=L).query_pairs(2 * a * (1 - 1e-6))) == 0
-    d = x1 - c
-    d -= L * np.round(d / L)
-    assert np.linalg.norm(d, axis=1).min() >= 1 + 2 * a - 1e-9
-    assert np.abs(x1 - x0).max() > 0.01
