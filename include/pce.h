@@ -57,6 +57,10 @@ typedef enum {
 /* pce_params.flags */
 #define PCE_FLAG_NO_PRECOND 1  /* plain (unpreconditioned) conjugate gradients in pce_solve */
 #define PCE_FLAG_CUFFT_3D   2  /* 3-D cuFFT plans + separate scaling pass instead of 2-D cuFFT per plane + fused z pass */
+#define PCE_FLAG_FIELD_IK   4  /* field mode of pce_evaluate / pce_forces: ik differentiation in wave space (E_d from the inverse
+                                  transform of -i k_d times the scaled spectrum, gathered with the plain window: three more inverse
+                                  transforms, wave-space momentum conserved to rounding) instead of the gradient of the gather
+                                  window (default, one transform pair; reading A3). */
 
 /* Parameters of the spectral Ewald sum and of the solver.
  * eta is NOT a free input: eta = h^2 xi^2 P / pi (eq. 31,

@@ -98,7 +98,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     free_system(c);
     krylov_free(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -407,9 +407,22 @@ static int apply_operator(pce_ctx* c, Bins& sr, Bins& sw, Bins& tr, Bins& tw, bo
     else rc = real_direct(c, tr, sr, field, c->w_real, c->w_ex, c->w_ey, c->w_ez);          // step 1, eq. 20-21
     if (rc) return rc;
     if ((rc = c->use_cols ? wave_spread_cols(c, sw) : wave_spread_bricks(c, sw))) return rc;  // step 2, eq. 25
-    if ((rc = wave_fft_scale_ifft(c))) return rc;                                        // steps 3-5, eq. 26
-    if ((rc = c->use_cols ? wave_gather_cols(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz)
-                          : wave_gather_bricks(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    if (field && (c->p.flags & PCE_FLAG_FIELD_IK)) {
+        // ik differentiation ("potential and its gradients"): E_d = IFFT[-i k_d G H^] gathered with the plain
+        // window -- three more inverse transforms and gathers, but the wave-space forces then sum to zero to rounding
+        if ((rc = wave_forward(c))) return rc;                                           // step 3
+        double* dst[4] = {c->w_kx, c->w_ky, c->w_kz, c->w_wave};
+        for (int k = 0; k < 4; ++k) {
+            if ((rc = wave_scale_inverse(c, k < 3 ? k : -1))) return rc;                 // steps 4-5, eq. 26 (times -i k_d)
+            if ((rc = c->use_cols ? wave_gather_cols(c, tw, false, dst[k], nullptr, nullptr, nullptr)
+                                  : wave_gather_bricks(c, tw, false, dst[k], nullptr, nullptr, nullptr))) return rc;  // step 6
+            if (k < 3) c->tm.n_fft_pairs++;
+        }
+    } else {
+        if ((rc = wave_fft_scale_ifft(c))) return rc;                                    // steps 3-5, eq. 26
+        if ((rc = c->use_cols ? wave_gather_cols(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz)
+                              : wave_gather_bricks(c, tw, field, c->w_wave, c->w_kx, c->w_ky, c->w_kz))) return rc;  // step 6, eq. 27
+    }
     {
         PassTimer t(c, PASS_OTHER);
         k_finalize<<<cdiv(n, 256), 256, 0, c->st>>>(n, tr.inv, tw.inv, c->w_real, c->w_wave, c->scal, c->kconst, psi, field ? 1 : 0,

@@ -141,6 +141,7 @@ struct pce_ctx {
     // mesh
     double* grid = nullptr;
     cufftDoubleComplex* gridk = nullptr;
+    cufftDoubleComplex* gridk2 = nullptr;  // second half spectrum (ik-differentiated fields: the forward spectrum is used four times)
     cufftHandle planF = 0, planB = 0;
     void* fft_work = nullptr;
     bool have_plans = false;
@@ -267,11 +268,13 @@ void chebtab_build(double s_lo, double s_hi, long double (*f)(long double, const
 
 // wave.cu
 int wave_fft_scale_ifft(pce_ctx* c);
+int wave_forward(pce_ctx* c);                 // mesh -> (x, y)-transformed half spectrum (or the full 3-D transform)
+int wave_scale_inverse(pce_ctx* c, int deriv);  // Green's function (times -i k_d if deriv >= 0) and back to the mesh; the forward spectrum is kept when deriv >= 0
 
 // zfft.cu
 bool zfft_supported(const pce_params& p);
 int zfft_init(pce_ctx* c);
-int zfft_scale(pce_ctx* c);
+int zfft_scale(pce_ctx* c, const void* in, void* out, int deriv);  // deriv = -1: potential; 0..2: times -i k_d (field component d)
 
 // wave_bricks.cu
 int wave_bricks_init(pce_ctx* c);

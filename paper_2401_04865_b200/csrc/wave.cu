@@ -14,7 +14,7 @@
 // two divisions: ~150 fp64 instructions) and applies it to the up to four mirror points (+-ky, +-kz) of the
 // half spectrum: the pass is then bound by its 32 bytes per complex mesh point of HBM traffic, not by the fp64 pipe.
 __global__ void __launch_bounds__(256)
-k_scale(WaveConst wc, cufftDoubleComplex* __restrict__ gk, const int* __restrict__ skip)
+k_scale(WaveConst wc, const cufftDoubleComplex* gin, cufftDoubleComplex* gout, int deriv, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     const int nxh = wc.Nxh, ny = wc.Ng[1], nz = wc.Ng[2];
@@ -33,45 +33,76 @@ k_scale(WaveConst wc, cufftDoubleComplex* __restrict__ gk, const int* __restrict
             const double j0 = (ka < 1e-4) ? 1.0 - ka * ka * (1.0 / 6.0) : sin(ka) / ka;
             f = wc.scale_norm * j0 * j0 * exp(-(wc.gexp[0] * kx2 + wc.gexp[1] * ky2 + wc.gexp[2] * kz2)) / k2;
         }
+        // ik differentiation (deriv = 0, 1, 2): times -i k_d, k_d signed (the mirror rows carry -k_y, -k_z), 0 at the Nyquist mode
+        double kd = 0.0;
+        if (deriv == 0) kd = (2 * ix == wc.Ng[0]) ? 0.0 : kx;
+        if (deriv == 1) kd = (2 * iy == ny) ? 0.0 : ky;
+        if (deriv == 2) kd = (2 * iz == nz) ? 0.0 : kz;
         const int my = (iy == 0 || 2 * iy == ny) ? -1 : ny - iy;  // mirror rows (none for the self-mirrored planes)
         const int mz = (iz == 0 || 2 * iz == nz) ? -1 : nz - iz;
-        cufftDoubleComplex* p00 = gk + ((size_t)iz * ny + iy) * nxh + ix;
-        cufftDoubleComplex* p10 = (my >= 0) ? gk + ((size_t)iz * ny + my) * nxh + ix : nullptr;
-        cufftDoubleComplex* p01 = (mz >= 0) ? gk + ((size_t)mz * ny + iy) * nxh + ix : nullptr;
-        cufftDoubleComplex* p11 = (my >= 0 && mz >= 0) ? gk + ((size_t)mz * ny + my) * nxh + ix : nullptr;
-        cufftDoubleComplex v00 = *p00, v10 = {0, 0}, v01 = {0, 0}, v11 = {0, 0};
-        if (p10) v10 = *p10;
-        if (p01) v01 = *p01;
-        if (p11) v11 = *p11;
-        v00.x *= f; v00.y *= f;
-        *p00 = v00;
-        if (p10) { v10.x *= f; v10.y *= f; *p10 = v10; }
-        if (p01) { v01.x *= f; v01.y *= f; *p01 = v01; }
-        if (p11) { v11.x *= f; v11.y *= f; *p11 = v11; }
+        const size_t o00 = ((size_t)iz * ny + iy) * nxh + ix;
+        const size_t o10 = (my >= 0) ? ((size_t)iz * ny + my) * nxh + ix : o00;
+        const size_t o01 = (mz >= 0) ? ((size_t)mz * ny + iy) * nxh + ix : o00;
+        const size_t o11 = (my >= 0 && mz >= 0) ? ((size_t)mz * ny + my) * nxh + ix : o00;
+        cufftDoubleComplex v00 = gin[o00], v10 = {0, 0}, v01 = {0, 0}, v11 = {0, 0};
+        if (my >= 0) v10 = gin[o10];
+        if (mz >= 0) v01 = gin[o01];
+        if (my >= 0 && mz >= 0) v11 = gin[o11];
+        auto apply = [&](cufftDoubleComplex v, double sgn) {
+            cufftDoubleComplex r;
+            if (deriv < 0) { r.x = v.x * f; r.y = v.y * f; }
+            else { const double g = f * kd * sgn; r.x = v.y * g; r.y = -v.x * g; }  // -i k (x + i y) = k (y - i x)
+            return r;
+        };
+        const double sy = (deriv == 1) ? -1.0 : 1.0, sz = (deriv == 2) ? -1.0 : 1.0;
+        gout[o00] = apply(v00, 1.0);
+        if (my >= 0) gout[o10] = apply(v10, sy);
+        if (mz >= 0) gout[o01] = apply(v01, sz);
+        if (my >= 0 && mz >= 0) gout[o11] = apply(v11, sy * sz);
     }
 }
 
-int wave_fft_scale_ifft(pce_ctx* c)
+int wave_forward(pce_ctx* c)
 {
-    {
-        PassTimer t(c, PASS_FFT);
-        if (cufftExecD2Z(c->planF, c->grid, c->gridk) != CUFFT_SUCCESS) { c->err = "cufftExecD2Z failed"; return PCE_ECUFFT; }
+    PassTimer t(c, PASS_FFT);
+    if (cufftExecD2Z(c->planF, c->grid, c->gridk) != CUFFT_SUCCESS) { c->err = "cufftExecD2Z failed"; return PCE_ECUFFT; }
+    return PCE_OK;
+}
+
+// deriv < 0: in place on gridk; deriv >= 0: gridk -> gridk2 (the forward spectrum survives for the next component)
+int wave_scale_inverse(pce_ctx* c, int deriv)
+{
+    cufftDoubleComplex* out = c->gridk;
+    if (deriv >= 0) {
+        if (!c->gridk2) {
+            const size_t nk = (size_t)c->wk.Nxh * c->wk.Ng[1] * c->wk.Ng[2];
+            if (cudaMalloc(&c->gridk2, nk * sizeof(cufftDoubleComplex)) != cudaSuccess) { c->err = "out of device memory for the second spectrum (ik fields)"; return PCE_ENOMEM; }
+            c->bytes += (long long)(nk * 16); c->bytes_base += (long long)(nk * 16);
+        }
+        out = c->gridk2;
     }
     if (c->use_zfft) {
         PassTimer t(c, PASS_SCALE);  // z FFT + Green's function + inverse z FFT in one pass over the half spectrum
-        int rc = zfft_scale(c);
+        int rc = zfft_scale(c, c->gridk, out, deriv);
         if (rc) return rc;
     } else {
         PassTimer t(c, PASS_SCALE);
         const size_t total = (size_t)c->wk.Nxh * (c->wk.Ng[1] / 2 + 1) * (c->wk.Ng[2] / 2 + 1);
         const int blocks = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
-        k_scale<<<blocks, 256, 0, c->st>>>(c->wk, c->gridk, c->skip_flag);
+        k_scale<<<blocks, 256, 0, c->st>>>(c->wk, c->gridk, out, deriv, c->skip_flag);
         c->launches++;
         PCE_CUDA(c, cudaGetLastError());
     }
     {
         PassTimer t(c, PASS_IFFT);
-        if (cufftExecZ2D(c->planB, c->gridk, c->grid) != CUFFT_SUCCESS) { c->err = "cufftExecZ2D failed"; return PCE_ECUFFT; }
+        if (cufftExecZ2D(c->planB, out, c->grid) != CUFFT_SUCCESS) { c->err = "cufftExecZ2D failed"; return PCE_ECUFFT; }
     }
     return PCE_OK;
+}
+
+int wave_fft_scale_ifft(pce_ctx* c)
+{
+    int rc = wave_forward(c);
+    if (!rc) rc = wave_scale_inverse(c, -1);
+    return rc;
 }

@@ -35,14 +35,6 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// the same, issued only if `on` != 0 (warp-uniform): a predicated DMMA, no branch and no re-convergence code around it
-__device__ __forceinline__ void dmma884_if(unsigned on, double& d0, double& d1, double a, double b)
-{
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
-                 "@p mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n\t}"
-                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b), "r"(on));
-}
-
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -350,7 +342,10 @@ __device__ __forceinline__ void batch_weights(const WaveConst& wc, const double*
     zmask |= __shfl_xor_sync(0xffffffffu, zmask, 1);
     zmask |= __shfl_xor_sync(0xffffffffu, zmask, 2);
     if (GROUP == 8) zmask |= __shfl_xor_sync(0xffffffffu, zmask, 4);
-    if ((lane & (GROUP - 1)) == 0) s.mask[lane / GROUP] = (unsigned char)zmask;
+    // stored per PAIR of planes (bit k: plane 2k or 2k + 1 live): the kernels skip dead pairs by a jump table, because a
+    // predicated-off DMMA occupies the fp64 datapath exactly like a live one (measured) and short branches are if-converted
+    const unsigned pm = (zmask | (zmask >> 1)) & 0x55u;
+    if ((lane & (GROUP - 1)) == 0) s.mask[lane / GROUP] = (unsigned char)((pm & 1u) | ((pm >> 1) & 2u) | ((pm >> 2) & 4u) | ((pm >> 3) & 8u));
     __syncwarp();
 }
 
@@ -396,22 +391,27 @@ k_spread_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                 const double* w = s.wt + (live ? sb + t : 0) * STRIDE_PSI;
                 const double bx = live ? w[gq] : 0.0;        // B[t][gq] = wx_h[x = gq]
                 const double ay = live ? w[BR + gq] : 0.0;   // wy_h[y = gq]
-                const unsigned m = s.mask[sb >> 2];          // planes live for any hit of the group
-                if (m == 0xffu) {  // the common case: every plane live
-#pragma unroll
-                    for (int z = 0; z < BR; z += 2) {
-                        const double2 wz = *reinterpret_cast<const double2*>(w + 2 * BR + z);  // q_h wz_h[z], [z + 1]
-                        dmma884(acc[z][0], acc[z][1], ay * wz.x, bx);
-                        dmma884(acc[z + 1][0], acc[z + 1][1], ay * wz.y, bx);
-                    }
-                } else {
-#pragma unroll
-                    for (int z = 0; z < BR; z += 2) {
-                        const double2 wz = *reinterpret_cast<const double2*>(w + 2 * BR + z);
-                        dmma884_if(m & (1u << z), acc[z][0], acc[z][1], ay * wz.x, bx);
-                        dmma884_if(m & (2u << z), acc[z + 1][0], acc[z + 1][1], ay * wz.y, bx);
-                    }
+                const unsigned m = s.mask[sb >> 2];          // plane pairs live for any hit of the group
+#define SPREAD_PAIR(z)                                                                                   \
+    {                                                                                                    \
+        const double2 wz = *reinterpret_cast<const double2*>(w + 2 * BR + (z)); /* q_h wz_h[z], [z + 1] */ \
+        dmma884(acc[z][0], acc[z][1], ay * wz.x, bx);                                                    \
+        dmma884(acc[(z) + 1][0], acc[(z) + 1][1], ay * wz.y, bx);                                        \
+    }
+                switch (m) {  // the live pairs of a group are contiguous (supports are); anything else: all pairs (dead weights are 0)
+                    case 0x1: SPREAD_PAIR(0) break;
+                    case 0x3: SPREAD_PAIR(0) SPREAD_PAIR(2) break;
+                    case 0x7: SPREAD_PAIR(0) SPREAD_PAIR(2) SPREAD_PAIR(4) break;
+                    case 0x8: SPREAD_PAIR(6) break;
+                    case 0xc: SPREAD_PAIR(4) SPREAD_PAIR(6) break;
+                    case 0xe: SPREAD_PAIR(2) SPREAD_PAIR(4) SPREAD_PAIR(6) break;
+                    case 0x2: SPREAD_PAIR(2) break;
+                    case 0x4: SPREAD_PAIR(4) break;
+                    case 0x6: SPREAD_PAIR(2) SPREAD_PAIR(4) break;
+                    case 0x0: break;
+                    default: SPREAD_PAIR(0) SPREAD_PAIR(2) SPREAD_PAIR(4) SPREAD_PAIR(6) break;
                 }
+#undef SPREAD_PAIR
             }
             __syncwarp();
         }
@@ -511,35 +511,35 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                 const double* w = s.wt + (live ? hr : 0) * STRIDE;
                 const double a0 = live ? w[DW + t] : 0.0, a1 = live ? w[DW + t + 4] : 0.0;  // wy_h[y]
                 const double2 wx2 = *reinterpret_cast<const double2*>(w + 2 * t);           // wx_h[2t], [2t + 1]
-                const unsigned m = s.mask[sb >> 3];  // planes live for any hit of the group
+                const unsigned m = s.mask[sb >> 3];  // plane pairs live for any hit of the group
                 const int po = __shfl_sync(0xffffffffu, p_mine, hr & 31);
                 if (!FIELD) {
                     double u0 = 0.0, u1 = 0.0;
-                    if (m == 0xffu) {  // the common case: every plane live
-#pragma unroll
-                        for (int z = 0; z < BR; z += 2) {
-                            const double2 wz = *reinterpret_cast<const double2*>(w + 2 * DW + z);
-                            double t0 = 0.0, t1 = 0.0, s0 = 0.0, s1 = 0.0;
-                            dmma884(t0, t1, a0, H[z][0]);
-                            dmma884(t0, t1, a1, H[z][1]);
-                            dmma884(s0, s1, a0, H[z + 1][0]);
-                            dmma884(s0, s1, a1, H[z + 1][1]);
-                            u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);
-                            u0 = fma(wz.y, s0, u0); u1 = fma(wz.y, s1, u1);
-                        }
-                    } else {
-#pragma unroll
-                        for (int z = 0; z < BR; z += 2) {
-                            const double2 wz = *reinterpret_cast<const double2*>(w + 2 * DW + z);
-                            double t0 = 0.0, t1 = 0.0, s0 = 0.0, s1 = 0.0;  // dead planes: the products stay 0
-                            dmma884_if(m & (1u << z), t0, t1, a0, H[z][0]);
-                            dmma884_if(m & (1u << z), t0, t1, a1, H[z][1]);
-                            dmma884_if(m & (2u << z), s0, s1, a0, H[z + 1][0]);
-                            dmma884_if(m & (2u << z), s0, s1, a1, H[z + 1][1]);
-                            u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);
-                            u0 = fma(wz.y, s0, u0); u1 = fma(wz.y, s1, u1);
-                        }
+#define GATHER_PAIR(z)                                                                       \
+    {                                                                                        \
+        const double2 wz = *reinterpret_cast<const double2*>(w + 2 * DW + (z));              \
+        double t0 = 0.0, t1 = 0.0, s0 = 0.0, s1 = 0.0;                                       \
+        dmma884(t0, t1, a0, H[z][0]);                                                        \
+        dmma884(t0, t1, a1, H[z][1]);                                                        \
+        dmma884(s0, s1, a0, H[(z) + 1][0]);                                                  \
+        dmma884(s0, s1, a1, H[(z) + 1][1]);                                                  \
+        u0 = fma(wz.x, t0, u0); u1 = fma(wz.x, t1, u1);                                      \
+        u0 = fma(wz.y, s0, u0); u1 = fma(wz.y, s1, u1);                                      \
+    }
+                    switch (m) {  // live plane pairs of the group (contiguous); anything else: all pairs (dead weights are 0)
+                        case 0x1: GATHER_PAIR(0) break;
+                        case 0x3: GATHER_PAIR(0) GATHER_PAIR(2) break;
+                        case 0x7: GATHER_PAIR(0) GATHER_PAIR(2) GATHER_PAIR(4) break;
+                        case 0x8: GATHER_PAIR(6) break;
+                        case 0xc: GATHER_PAIR(4) GATHER_PAIR(6) break;
+                        case 0xe: GATHER_PAIR(2) GATHER_PAIR(4) GATHER_PAIR(6) break;
+                        case 0x2: GATHER_PAIR(2) break;
+                        case 0x4: GATHER_PAIR(4) break;
+                        case 0x6: GATHER_PAIR(2) GATHER_PAIR(4) break;
+                        case 0x0: break;
+                        default: GATHER_PAIR(0) GATHER_PAIR(2) GATHER_PAIR(4) GATHER_PAIR(6) break;
                     }
+#undef GATHER_PAIR
                     double r = fma(wx2.y, u1, wx2.x * u0);
                     r += __shfl_xor_sync(0xffffffffu, r, 1);
                     r += __shfl_xor_sync(0xffffffffu, r, 2);
@@ -548,19 +548,34 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                     const double b0 = live ? w[DW + BR + t] : 0.0, b1 = live ? w[DW + BR + t + 4] : 0.0;  // wy u_y
                     const double2 wxu2 = *reinterpret_cast<const double2*>(w + BR + 2 * t);               // wx u_x
                     double u0 = 0.0, u1 = 0.0, uz0 = 0.0, uz1 = 0.0, uy0 = 0.0, uy1 = 0.0;
-#pragma unroll
-                    for (int z = 0; z < BR; ++z) {
-                        const double wz = w[2 * DW + z], wzu = w[2 * DW + BR + z];
-                        double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;
-                        const unsigned on = m & (1u << z);
-                        dmma884_if(on, t0, t1, a0, H[z][0]);
-                        dmma884_if(on, t0, t1, a1, H[z][1]);
-                        dmma884_if(on, v0, v1, b0, H[z][0]);
-                        dmma884_if(on, v0, v1, b1, H[z][1]);
-                        u0 = fma(wz, t0, u0); u1 = fma(wz, t1, u1);
-                        uz0 = fma(wzu, t0, uz0); uz1 = fma(wzu, t1, uz1);
-                        uy0 = fma(wz, v0, uy0); uy1 = fma(wz, v1, uy1);
+#define GATHER_PLANE_F(z)                                                                    \
+    {                                                                                        \
+        const double wz = w[2 * DW + (z)], wzu = w[2 * DW + BR + (z)];                       \
+        double t0 = 0.0, t1 = 0.0, v0 = 0.0, v1 = 0.0;                                       \
+        dmma884(t0, t1, a0, H[z][0]);                                                        \
+        dmma884(t0, t1, a1, H[z][1]);                                                        \
+        dmma884(v0, v1, b0, H[z][0]);                                                        \
+        dmma884(v0, v1, b1, H[z][1]);                                                        \
+        u0 = fma(wz, t0, u0); u1 = fma(wz, t1, u1);                                          \
+        uz0 = fma(wzu, t0, uz0); uz1 = fma(wzu, t1, uz1);                                    \
+        uy0 = fma(wz, v0, uy0); uy1 = fma(wz, v1, uy1);                                      \
+    }
+#define GATHER_PAIR_F(z) GATHER_PLANE_F(z) GATHER_PLANE_F((z) + 1)
+                    switch (m) {
+                        case 0x1: GATHER_PAIR_F(0) break;
+                        case 0x3: GATHER_PAIR_F(0) GATHER_PAIR_F(2) break;
+                        case 0x7: GATHER_PAIR_F(0) GATHER_PAIR_F(2) GATHER_PAIR_F(4) break;
+                        case 0x8: GATHER_PAIR_F(6) break;
+                        case 0xc: GATHER_PAIR_F(4) GATHER_PAIR_F(6) break;
+                        case 0xe: GATHER_PAIR_F(2) GATHER_PAIR_F(4) GATHER_PAIR_F(6) break;
+                        case 0x2: GATHER_PAIR_F(2) break;
+                        case 0x4: GATHER_PAIR_F(4) break;
+                        case 0x6: GATHER_PAIR_F(2) GATHER_PAIR_F(4) break;
+                        case 0x0: break;
+                        default: GATHER_PAIR_F(0) GATHER_PAIR_F(2) GATHER_PAIR_F(4) GATHER_PAIR_F(6) break;
                     }
+#undef GATHER_PAIR_F
+#undef GATHER_PLANE_F
                     double r0 = fma(wx2.y, u1, wx2.x * u0);      // psi
                     double r1 = fma(wxu2.y, u1, wxu2.x * u0);    // sum W u_x H
                     double r2 = fma(wx2.y, uy1, wx2.x * uy0);    // sum W u_y H

@@ -137,8 +137,11 @@ __device__ __forceinline__ double shape_eval(const double* __restrict__ tab, int
 }
 
 // last forward stage x Green's function x first inverse stage on the tile column sp (stride KP), in place
+// deriv = 0, 1, 2: additionally multiply by -i k_d (ik differentiation: the field component E_d = -d psi / d x_d in wave
+// space); kxy = k_x or k_y of the thread's pencil (0 at the Nyquist mode), kzfac = 2 pi / L_z
 template <int N, int R>
-__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs);
+__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs,
+                                             int deriv, double kxy, double kzfac);
 
 template <int N> struct Radices {
     static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;  // N = 8^m * rest
@@ -149,7 +152,8 @@ template <int N> struct Radices {
 // KP pencils per CTA, N/8 threads per pencil.  zexp = [ex | ey | ez]: exp(-gexp_d k_d^2) per axis (host tables).
 constexpr int KP = 4;
 template <int N, int R>
-__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs)
+__device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const double2* __restrict__ tw, const double* __restrict__ gs,
+                                             int deriv, double kxy, double kzfac)
 {
     constexpr int NB = 8 / R, NTH = N / 8;
     double2 v[8];
@@ -166,8 +170,13 @@ __device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const do
         twiddle_dft<R, -1>(v + q * R, b, tw);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const double gf = gs[(b + r * (N / R)) * KP + p];
+            const int iz = b + r * (N / R);
+            const double gf = gs[iz * KP + p];
             v[q * R + r].x *= gf; v[q * R + r].y *= gf;
+            if (deriv >= 0) {  // -i k_d (x + i y) = k_d (y - i x); the Nyquist mode has no derivative on an even mesh
+                const double kd = (deriv == 2) ? kzfac * (double)(iz < N / 2 ? iz : (iz == N / 2 ? 0 : iz - N)) : kxy;
+                v[q * R + r] = make_double2(v[q * R + r].y * kd, -v[q * R + r].x * kd);
+            }
         }
         dftR<R, +1>(v + q * R);  // Ns = 1: no twiddles; outputs at b R + r
 #pragma unroll
@@ -176,7 +185,7 @@ __device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const do
 }
 template <int N>
 __global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
-k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
+k_zfft_scale(WaveConst wc, const double2* gin, double2* gout, int deriv, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
              const double* __restrict__ shape, int shape_key_lo, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -214,18 +223,22 @@ k_zfft_scale(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__
     for (int pass = 0; pass < 2; ++pass) {
         const int y = pass == 0 ? iy : my;
         if (y < 0) break;
-        double2* col = gk + (size_t)y * nxh + (col_ok ? kxi : 0);
+        const double2* cin = gin + (size_t)y * nxh + (col_ok ? kxi : 0);
+        double2* col = gout + (size_t)y * nxh + (col_ok ? kxi : 0);
         double2* sp = tile + p;
+        double kxy = 0.0;
+        if (deriv == 0) kxy = (2 * kxi == wc.Ng[0]) ? 0.0 : wc.kfac[0] * kxi;
+        if (deriv == 1) kxy = (2 * iy == ny) ? 0.0 : wc.kfac[1] * (pass == 0 ? iy : -iy);
         __syncthreads();  // twiddles and Green's function stored / previous pass done with the tile
         // ---- forward: the first stage reads global memory; all but the last stage of the transform here
-        stage<N, 8, -1, false>(col, zstr, col_ok, sp, KP, true, 1, j, tw, nullptr);
+        stage<N, 8, -1, false>(cin, zstr, col_ok, sp, KP, true, 1, j, tw, nullptr);
         __syncthreads();
         int Ns = 8;
         if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         // ---- last forward stage (radix REST, Ns = N / REST) x Green's function x first inverse stage (radix REST, Ns = 1), in
         // registers: the forward stage leaves element b + r N/REST in slot r, which is what the inverse stage reads
-        fused_middle<N, REST>(sp, j, p, tw, gs);
+        fused_middle<N, REST>(sp, j, p, tw, gs, deriv, kxy, wc.kfac[2]);
         __syncthreads();
         // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
         Ns = REST;
@@ -329,7 +342,7 @@ k_zfft_scale_pipe(WaveConst wc, double2* __restrict__ gk, const double2* __restr
         if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
         // ---- last forward stage x Green's function x first inverse stage, in registers
-        fused_middle<N, REST>(sp, j, p, tw, gs);
+        fused_middle<N, REST>(sp, j, p, tw, gs, -1, 0.0, 0.0);
         __syncthreads();
         // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
         Ns = REST;
@@ -360,7 +373,7 @@ template <int N> int launch_pipe(pce_ctx* c)
     return PCE_OK;
 }
 
-template <int N> int launch(pce_ctx* c)
+template <int N> int launch(pce_ctx* c, const double2* gin, double2* gout, int deriv)
 {
     const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
     if (!c->zfft_attr_set && smem > 48 * 1024) {  // the attribute is per device: once per context, not per process
@@ -368,8 +381,7 @@ template <int N> int launch(pce_ctx* c)
         c->zfft_attr_set = true;
     }
     const dim3 grid(cdiv(c->wk.Nxh, KP), c->wk.Ng[1] / 2 + 1);
-    k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp, c->zshape,
-                                                        c->zshape_key_lo, c->skip_flag);
+    k_zfft_scale<N><<<grid, N / 8 * KP, smem, c->st>>>(c->wk, gin, gout, deriv, c->ztw, c->zexp, c->zshape, c->zshape_key_lo, c->skip_flag);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -421,10 +433,12 @@ int zfft_init(pce_ctx* c)
     return PCE_OK;
 }
 
-int zfft_scale(pce_ctx* c)
+int zfft_scale(pce_ctx* c, const void* in, void* out, int deriv)
 {
+    const double2* gin = static_cast<const double2*>(in);
+    double2* gout = static_cast<double2*>(out);
     static const bool pipe = [] { const char* e = getenv("PCE_ZFFT_PIPE"); return e && e[0] == '1'; }();
-    if (pipe) {  // pipelined variant (persistent CTAs, cp.async double buffer): measured slower on B200 (fewer resident warps), kept for experiments
+    if (pipe && deriv < 0 && in == out && in == (const void*)c->gridk) {  // pipelined variant (persistent CTAs, cp.async double buffer): measured slower on B200 (fewer resident warps), kept for experiments
         switch (c->p.Ng[2]) {
             case 64: return launch_pipe<64>(c);
             case 128: return launch_pipe<128>(c);
@@ -435,13 +449,13 @@ int zfft_scale(pce_ctx* c)
         }
     }
     switch (c->p.Ng[2]) {
-        case 16: return launch<16>(c);
-        case 32: return launch<32>(c);
-        case 64: return launch<64>(c);
-        case 128: return launch<128>(c);
-        case 256: return launch<256>(c);
-        case 512: return launch<512>(c);
-        case 1024: return launch<1024>(c);
+        case 16: return launch<16>(c, gin, gout, deriv);
+        case 32: return launch<32>(c, gin, gout, deriv);
+        case 64: return launch<64>(c, gin, gout, deriv);
+        case 128: return launch<128>(c, gin, gout, deriv);
+        case 256: return launch<256>(c, gin, gout, deriv);
+        case 512: return launch<512>(c, gin, gout, deriv);
+        case 1024: return launch<1024>(c, gin, gout, deriv);
         default: c->err = "zfft_scale: unsupported N_z"; return PCE_EINVAL;
     }
 }

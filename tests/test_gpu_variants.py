@@ -1,0 +1,109 @@
+"""SURVEY.md 8(f) f4 variants on the device: ik-differentiated fields (PCE_FLAG_FIELD_IK) and rod-like "fiber"
+bodies of four bead lines, each against the oracle at the north-star bars."""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+from conftest import body_vector_error
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def _E(out):
+    import torch
+    return torch.stack(out[1:], dim=1).cpu().numpy()
+
+
+@pytest.mark.parametrize("fused_z", [True, False])
+def test_ik_field_mode_matches_the_oracle_and_conserves_momentum(fused_z):
+    """E from -i k times the scaled spectrum: parity <= 1e-9 with the oracle (and so with the window-gradient mode), and the
+    total electrostatic force sum_a q_a E_a vanishes to rounding -- spread and gather use the same window, the ik multiplier is
+    odd in k -- which the window-gradient mode only does to the Ewald tolerance."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.config2(d=2.4)
+    rng = np.random.default_rng(5)
+    q = rng.normal(size=w.N)
+    q -= q.mean()
+    psi_o, E_o = orc.ewald_eval(w.x, q, w.L, w.a)
+    tot = {}
+    for ik in (True, False):
+        ctx = pce.context_for(w, field_ik=ik, fused_z=fused_z)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        out = ctx.evaluate(torch.from_numpy(q).cuda())
+        psi, E = out[0].cpu().numpy(), _E(out)
+        assert rel(psi, psi_o) < 1e-9 and rel(E, E_o) < 1e-9, (ik, rel(psi, psi_o), rel(E, E_o))
+        tot[ik] = np.abs((q[:, None] * E).sum(axis=0)).max() / np.abs(q[:, None] * E).sum(axis=0).max()
+        ctx.close()
+    assert tot[True] < 1e-13, tot
+    assert tot[True] < 0.05 * tot[False], tot
+
+
+def test_ik_field_mode_in_a_rectangular_box_and_through_the_solve():
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.tiny_random(seed=21, n_body=2, n_ion=40, L=6.0, Ng=32)
+    w.L = np.array([6.0, 7.5, 9.0])
+    w.Ng = np.array([32, 40, 48])          # N_z = 48: the 3-D cuFFT path with the separate scaling pass
+    ctx = pce.context_for(w, field_ik=True)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+    oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, Phi_body=Phio)
+    assert rel(q.cpu().numpy(), qo) < 1e-9 and rel(out["f"].cpu().numpy(), oo["f"]) < 1e-8
+    assert body_vector_error(out["F"].cpu().numpy(), oo["F"], oo["f"])[0] < 1e-8
+    assert body_vector_error(out["T"].cpu().numpy(), oo["T"], oo["f"])[0] < 1e-8
+    ctx.close()
+
+
+@pytest.mark.parametrize("chi", [5, 10])
+def test_fiber_dipole_and_torque_versus_angle(chi):
+    """Fig. 4 of the paper as a parity case: dipole and torque of a four-line fiber at 0, 30, 45, 90 degrees to the field."""
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    for deg in (0, 30, 45, 90):
+        w = wl.fiber_in_field(chi=chi, theta=np.deg2rad(deg), Ng=64 if chi == 5 else 96)
+        ctx = pce.context_for(w)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        q, Phi, info = ctx.solve(Q, qi, w.E0)
+        assert info["converged"]
+        out = ctx.forces(q, w.E0)
+        qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+        oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, Phi_body=Phio)
+        assert rel(q.cpu().numpy(), qo) < 1e-9, (deg, rel(q.cpu().numpy(), qo))
+        assert rel(out["S"].cpu().numpy(), oo["S"]) < 1e-9
+        assert rel(out["f"].cpu().numpy(), oo["f"]) < 1e-8
+        eT, kind = body_vector_error(out["T"].cpu().numpy(), oo["T"], oo["f"])
+        assert eT < 1e-8, (deg, eT, kind)
+        if deg in (30, 45):
+            assert kind == "rel" and out["T"][0, 1].item() < 0      # a real torque, towards alignment with E0
+        ctx.close()
+
+
+def test_fiber_with_ions_full_parity():
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.fiber_in_field(chi=10, theta=0.6, n_ion=400, Ng=96)
+    ctx = pce.context_for(w)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    out = ctx.forces(q, w.E0)
+    qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+    oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, Phi_body=Phio)
+    assert rel(q.cpu().numpy(), qo) < 1e-9 and rel(out["psi"].cpu().numpy(), oo["psi"]) < 1e-9
+    assert rel(out["f"].cpu().numpy(), oo["f"]) < 1e-8
+    assert body_vector_error(out["F"].cpu().numpy(), oo["F"], oo["f"])[0] < 1e-8
+    assert body_vector_error(out["T"].cpu().numpy(), oo["T"], oo["f"])[0] < 1e-8
+    ctx.close()

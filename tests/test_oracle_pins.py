@@ -470,3 +470,33 @@ def test_effective_permittivity_matches_the_constrained_solves_and_dilute_limit(
     phi_eff = (e1[2, 2] - 1) / (e1[2, 2] + 2)  # invert Clausius-Mossotti: phi = (eps - 1)/(eps + 2)
     phi_geo = 4 * np.pi / 3 / 8.0 ** 3
     assert 1.0 < phi_eff / phi_geo < 1.25  # effective radius a few per cent above the geometric one
+
+
+def test_fiber_torque_follows_the_angle_law_of_an_axisymmetric_polarizable_body():
+    """PAPER.md:348 (Fig. 4): for a slender body with polarizability alpha_par along its axis and alpha_perp across it the dipole
+    is S = alpha_perp E0 + (alpha_par - alpha_perp)(n.E0) n, hence S.E0 = alpha_perp + (alpha_par - alpha_perp) cos^2 theta and
+    |T| = |S x E0| = (alpha_par - alpha_perp) sin(2 theta) / 2: no torque at 0 and 90 degrees, maximum at 45, sense towards
+    alignment.  Linear response of eq. 13 fixes these laws exactly for an isolated body; the periodic images of a large box
+    perturb them at the 1e-2 level."""
+    import workloads as wl
+    res = {}
+    for deg in (0, 30, 45, 60, 90):
+        w = wl.fiber_in_field(chi=5, theta=np.deg2rad(deg), L=30.0)
+        q, Phi, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+        o = orc.forces_torques(w.x, w.body_offset, q, w.E0, w.L, w.a, Phi_body=Phi)
+        res[deg] = (o["S"][0], o["T"][0], o["F"][0])
+    a_par, a_perp = res[0][0][2], res[90][0][2]
+    assert a_par > 3 * a_perp > 0                                  # a slender conductor polarizes along its axis
+    tscale = 0.5 * (a_par - a_perp)
+    for deg in (0, 90):
+        assert np.abs(res[deg][1]).max() < 1e-9 * tscale            # symmetric positions: no torque
+    for deg in (30, 45, 60):
+        S, T, F = res[deg]
+        th = np.deg2rad(deg)
+        assert abs(S[2] - (a_perp + (a_par - a_perp) * np.cos(th) ** 2)) < 2e-2 * a_par
+        assert abs(T[0]) < 1e-9 * tscale and abs(T[2]) < 1e-9 * tscale
+        assert T[1] < 0                                             # the axis (sin th, 0, cos th) turns towards E0 = e_z
+        assert abs(-T[1] - tscale * np.sin(2 * th)) < 3e-2 * tscale
+        assert np.allclose(T, np.cross(S, w.E0), atol=3e-2 * tscale)  # isolated body: T = S x E0 (PAPER.md:348)
+        assert np.abs(F).max() < 1e-9 * tscale                      # no net force in a uniform field on a neutral body
+    assert -res[45][1][1] > -res[30][1][1] and -res[45][1][1] > -res[60][1][1]

@@ -64,3 +64,27 @@ def test_config5_replica_self_checks():
     t = geo.fibonacci_spheroid(1000)
     d, _ = cKDTree(t).query(t, k=2)
     assert d[:, 1].max() / d[:, 1].min() < 1.6
+
+
+def test_fiber_generator():
+    """Four touching bead lines: 8 chi beads, nearest neighbours exactly 2a apart, length / width = chi."""
+    import numpy as np
+    from scipy.spatial import cKDTree
+    import workloads as wl
+    from workloads import geometry as geo
+    for chi in (5, 10):
+        m = geo.fiber(chi, a=0.3)
+        assert m.shape == (8 * chi, 3) and np.allclose(m.mean(axis=0), 0)
+        d, _ = cKDTree(m).query(m, k=2)
+        assert np.allclose(d[:, 1], 0.6)
+        ext = m.max(axis=0) - m.min(axis=0) + 0.6
+        assert np.isclose(ext[2] / ext[0], chi) and np.isclose(ext[0], ext[1])
+    w = wl.fiber_in_field(chi=5, theta=np.pi / 3)
+    X = w.x[:w.N_bead].mean(axis=0)
+    axis = w.x[w.N_bead // 4 - 1] - w.x[0]  # first line, first to last bead
+    axis /= np.linalg.norm(axis)
+    assert np.allclose(X, w.L / 2) and np.isclose(axis @ w.E0, np.cos(np.pi / 3))
+    wi = wl.fiber_in_field(chi=5, n_ion=50)
+    assert wi.N_ion == 50 and abs(wi.q_ion.sum()) < 1e-12
+    dmin, _ = cKDTree(wi.x[:wi.N_bead]).query(wi.x[wi.N_bead:], k=1)
+    assert dmin.min() >= 2.5 * wi.a

@@ -245,4 +245,30 @@ def tiny_random(seed=7, n_body=2, n_bead_side=1, n_ion=6, L=6.0, Ng=32, a=0.2, n
     return _mk("tiny_random", beads, off, Q, ions, qion, rng.normal(size=3), L, Ng, a, centres=np.array(centres))
 
 
+def fiber_in_field(chi=5, theta=0.25 * np.pi, L=None, Ng=64, a=0.25, n_ion=0, seed=BASE_SEED + 7):
+    """One rigid fiber of aspect ratio chi (four bead lines) at the box centre, its long axis in the (x, z) plane at
+    angle theta to the applied field E0 = (0, 0, 1) (Fig. 4), optionally with ions around it."""
+    rng = np.random.default_rng(seed)
+    m = geo.fiber(chi, a)
+    half = 2.0 * a * chi
+    if L is None:
+        L = 4.0 * half + 8.0 * a
+    c, s = np.cos(theta), np.sin(theta)
+    Rot = np.array([[c, 0.0, s], [0.0, 1.0, 0.0], [-s, 0.0, c]])  # about y: the axis e_z goes to (sin theta, 0, cos theta)
+    centre = np.full(3, L / 2)
+    beads = m @ Rot.T + centre
+    if n_ion:
+        from scipy.spatial import cKDTree
+        tree = cKDTree(beads)
+
+        def keep(p):
+            d, _ = tree.query(p, k=1, distance_upper_bound=2.5 * a)
+            return ~np.isfinite(d)
+        ions = geo.place_ions(rng, n_ion, L, 2 * a, keep)
+        qion = np.concatenate([np.ones(n_ion // 2), -np.ones(n_ion - n_ion // 2)])
+    else:
+        ions, qion = np.zeros((0, 3)), []
+    return _mk(f"fiber_chi{chi}", beads, [0, len(m)], np.zeros(1), ions, qion, [0, 0, 1.0], L, Ng, a, theta=theta, chi=chi)
+
+
 ALL = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}

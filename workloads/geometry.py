@@ -114,3 +114,13 @@ def place_ions(rng, n, L, min_sep, keep_mask_fn, oversample=1.3, max_rounds=50):
     if acc.shape[0] < n:
         raise RuntimeError("ion placement did not converge")
     return acc[:n]
+
+
+def fiber(chi: int, a: float = 1.0) -> np.ndarray:
+    """The paper's "fiber": four parallel lines of touching beads of radius a, the lines through the corners of a
+    square of side 2a (neighbouring lines touch), 2 chi beads per line at spacing 2a along z -- length 4 a chi over width 4a,
+    i.e. ratio of the longest to the shortest axis chi (reading B8).  Centred at the origin; (8 chi, 3)."""
+    n = 2 * int(chi)
+    z = (np.arange(n) - 0.5 * (n - 1)) * 2.0 * a
+    pts = [np.stack([np.full(n, sx * a), np.full(n, sy * a), z], axis=1) for sx in (-1.0, 1.0) for sy in (-1.0, 1.0)]
+    return np.concatenate(pts)
