@@ -134,6 +134,12 @@ int pce_set_system(pce_ctx* ctx, int N, int N_body, const int* body_offset,
 /* New positions for the same system (e.g. next time step). */
 int pce_set_positions(pce_ctx* ctx, const double* x, const double* y, const double* z);
 
+/* Reference points X_i of the bodies (device X, Y, Z of length N_body) in place of the bead means: r_ij becomes the minimum
+ * image of x_ij - X_i (eq. 12; the paper says "centre of mass").  The induced charges do not depend
+ * on the choice (a shift d of X_i changes r_ij.E0 by a constant per body, absorbed by Phi_i -> Phi_i + d.E0); S_i, T_i, Psi_i
+ * and U_i are then taken about the new point.  Valid until the next pce_set_positions / pce_set_system / pce_bd_step. */
+int pce_set_centres(pce_ctx* ctx, const double* X, const double* Y, const double* Z);
+
 /* psi = M_bb q over the N_bead conductor beads only (the solver's matvec;
  * eq. 8, restricted to bead sources and bead targets).
  * q, psi: device, length N_bead, caller order. */
@@ -161,6 +167,9 @@ int pce_evaluate(pce_ctx* ctx, const double* q, double* psi,
  * positions only, so it is built once in pce_set_system and stays valid while
  * pce_set_positions moves the bodies rigidly; a non-rigid
  * update costs iterations, never accuracy (the solution of eq. 13 is unique).
+ * GMRES on the indefinite saddle-point form of eq. 13 (the paper's ref. 51 is GMRES-based) is not offered: M is
+ * symmetric positive definite, the projected system is SPD, its solution is the unique solution of eq. 13, and
+ * CG needs one vector of history and two fixed-order dot products per iteration where GMRES needs a growing basis.
  * Returns PCE_ENOCONV if max_iter was hit. */
 int pce_solve(pce_ctx* ctx, const double* Q_body, const double* q_ion, const double E0[3],
               int warm_start, double* q, double* Phi_body, pce_solve_info* info);

@@ -22,7 +22,7 @@ EXPORTS = (
     "pce_suggest_params", "pce_create", "pce_destroy", "pce_last_error", "pce_set_system", "pce_set_positions",
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
     "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks", "pce_debug_poison_shared_memory",
-    "pce_capacitance_columns", "pce_effective_permittivity", "pce_bd_step", "pce_radial_profile",
+    "pce_capacitance_columns", "pce_effective_permittivity", "pce_bd_step", "pce_radial_profile", "pce_set_centres",
 )
 
 
@@ -83,6 +83,7 @@ def load():
     lib.pce_last_error.restype = C.c_char_p
     lib.pce_set_system.argtypes = [vp, C.c_int, C.c_int, ip, vp, vp, vp]
     lib.pce_set_positions.argtypes = [vp, vp, vp, vp]
+    lib.pce_set_centres.argtypes = [vp, vp, vp, vp]
     lib.pce_matvec.argtypes = [vp, vp, vp]
     lib.pce_evaluate.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.pce_solve.argtypes = [vp, vp, vp, dp, C.c_int, vp, vp, C.POINTER(PceSolveInfo)]
@@ -212,6 +213,11 @@ class Context:
         for t in (x, y, z):
             self._chk(t, self.N)
         self._ck(self.lib.pce_set_positions(self.h, _ptr(x), _ptr(y), _ptr(z)))
+
+    def set_centres(self, X, Y, Z):
+        for t in (X, Y, Z):
+            self._chk(t, self.N_body)
+        self._ck(self.lib.pce_set_centres(self.h, _ptr(X), _ptr(Y), _ptr(Z)))
 
     # ---- operator
     def matvec(self, q):

@@ -60,6 +60,31 @@ int bodies_setup(pce_ctx* c)
     return PCE_OK;
 }
 
+// caller-supplied centres (pce_set_centres): r_ij = minimum image of x_ij - X_i
+__global__ void k_rel_to_centres(int nbead, const int* __restrict__ body_of, const double* __restrict__ x, const double* __restrict__ y,
+                                 const double* __restrict__ z, const double* __restrict__ X, const double* __restrict__ Y,
+                                 const double* __restrict__ Z, double Lx, double Ly, double Lz, double* __restrict__ rx,
+                                 double* __restrict__ ry, double* __restrict__ rz)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nbead) return;
+    const int b = body_of[j];
+    rx[j] = min_img(x[j] - X[b], Lx); ry[j] = min_img(y[j] - Y[b], Ly); rz[j] = min_img(z[j] - Z[b], Lz);
+}
+
+int bodies_set_centres(pce_ctx* c, const double* X, const double* Y, const double* Z)
+{
+    if (c->Nbody == 0) return PCE_OK;
+    PCE_CUDA(c, cudaMemcpyAsync(c->X, X, (size_t)c->Nbody * 8, cudaMemcpyDeviceToDevice, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(c->Y, Y, (size_t)c->Nbody * 8, cudaMemcpyDeviceToDevice, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(c->Z, Z, (size_t)c->Nbody * 8, cudaMemcpyDeviceToDevice, c->st));
+    k_rel_to_centres<<<cdiv(c->Nbead, 256), 256, 0, c->st>>>(c->Nbead, c->body_of, c->x, c->y, c->z, c->X, c->Y, c->Z, c->p.L[0], c->p.L[1],
+                                                            c->p.L[2], c->rx, c->ry, c->rz);
+    c->launches++;
+    PCE_CUDA(c, cudaGetLastError());
+    return PCE_OK;
+}
+
 // ---------------------------------------------------------------- Krylov solve, whole iteration on the device
 // Conjugate gradients for eq. 13 with the ions eliminated (one-bead bodies of fixed charge):
 //     P M_bb P q = P b  on  Sigma q = Q,   P = I - Sigma^T (Sigma Sigma^T)^-1 Sigma  (subtract the per-body mean),
@@ -137,12 +162,14 @@ k_resid_init(int nb, const int* __restrict__ off, const double* __restrict__ rx,
     __shared__ double sh[32];
     const int b = blockIdx.x;
     const int j0 = off[b], j1 = off[b + 1];
-    double s = 0.0;
-    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += psi0[j];
+    // per-body means of psi0 and of r.E0 (the latter is 0 for bead-mean centres, not for caller-supplied ones: pce_set_centres)
+    double s = 0.0, sr = 0.0;
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) { s += psi0[j]; sr += rx[j] * e0x + ry[j] * e0y + rz[j] * e0z; }
     const double mean = (j1 > j0) ? block_sum(s, sh) / (j1 - j0) : 0.0;
+    const double mean_re = (j1 > j0) ? block_sum(sr, sh) / (j1 - j0) : 0.0;
     double gg = 0.0, rf = 0.0, pp = 0.0;
     for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
-        const double re = rx[j] * e0x + ry[j] * e0y + rz[j] * e0z;  // sum_j r_ij = 0, so P(r.E0) = r.E0
+        const double re = rx[j] * e0x + ry[j] * e0y + rz[j] * e0z - mean_re;  // P(r.E0)
         const double p0 = psi0[j], pc = p0 - mean;
         const double v = re - pc;
         g[j] = v;
@@ -324,15 +351,16 @@ k_cg_update(int nb, const int* __restrict__ off, const double* __restrict__ p, c
     }
 }
 
-// Phi_i = <psi_ij - r_ij.E0>_i = <psi_ij>_i
+// Phi_i = <psi_ij - r_ij.E0>_i  (= <psi_ij>_i for bead-mean centres)
 __global__ void __launch_bounds__(BT)
-k_body_mean(const int* __restrict__ off, const double* __restrict__ v, double* __restrict__ out)
+k_body_mean(const int* __restrict__ off, const double* __restrict__ v, const double* __restrict__ rx, const double* __restrict__ ry,
+            const double* __restrict__ rz, double e0x, double e0y, double e0z, double* __restrict__ out)
 {
     __shared__ double sh[32];
     const int b = blockIdx.x;
     const int j0 = off[b], j1 = off[b + 1];
     double s = 0.0;
-    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += v[j];
+    for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) s += v[j] - (rx[j] * e0x + ry[j] * e0y + rz[j] * e0z);
     s = block_sum(s, sh);
     if (threadIdx.x == 0) out[b] = (j1 > j0) ? s / (j1 - j0) : 0.0;
 }
@@ -523,7 +551,7 @@ int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double
     if ((rc = run_iterations(c, &inf))) return rc;
     {
         PassTimer t(c, PASS_KRYLOV);
-        k_body_mean<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_psi, Phi);
+        k_body_mean<<<nb, BT, 0, c->st>>>(c->body_off, c->cg_psi, c->rx, c->ry, c->rz, E0[0], E0[1], E0[2], Phi);
         k_copy<<<cdiv(nbead, 256), 256, 0, c->st>>>(nbead, c->cg_q, q);
         c->launches += 2;
     }

@@ -98,7 +98,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     free_system(c);
     krylov_free(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape); cudaFree(c->xytw); cudaFree(c->xy_ctr);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -167,6 +167,8 @@ static int create_impl(pce_ctx* c)
         }
         int rcz = zfft_init(c);
         if (rcz) return rcz;
+        c->use_fftxy = fftxy_supported(p);
+        if (c->use_fftxy && (rcz = fftxy_init(c))) return rcz;
     } else if (cufftMakePlan3d(c->planF, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_D2Z, &wsF) != CUFFT_SUCCESS ||
                cufftMakePlan3d(c->planB, p.Ng[2], p.Ng[1], p.Ng[0], CUFFT_Z2D, &wsB) != CUFFT_SUCCESS) {
         c->err = "cuFFT cannot plan this grid";
@@ -327,6 +329,14 @@ extern "C" int pce_set_positions(pce_ctx* c, const double* x, const double* y, c
     int rc = positions_impl(c, x, y, z);
     timing_end(c);
     return rc;
+}
+
+extern "C" int pce_set_centres(pce_ctx* c, const double* X, const double* Y, const double* Z)
+{
+    if (!c) return PCE_EINVAL;
+    if (!c->have_system) { c->err = "pce_set_centres before pce_set_system"; return PCE_ESTATE; }
+    if (c->Nbody > 0 && (!X || !Y || !Z)) { c->err = "NULL centres"; return PCE_EINVAL; }
+    return bodies_set_centres(c, X, Y, Z);
 }
 
 // ---------------------------------------------------------------- the operator

@@ -150,6 +150,10 @@ struct pce_ctx {
     double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function
     double* zshape = nullptr;  // piecewise-polynomial table of the shape factor j0(ka)^2 / k^2 as a function of k^2
     int zshape_key_lo = 0, zshape_n = 0;
+    bool use_fftxy = false;    // own (x, y) transforms, one HBM trip per plane and direction (fftxy.cu) instead of cuFFT 2-D plans
+    double2* xytw = nullptr;   // twiddles exp(-2 pi i m / N_x)
+    int* xy_ctr = nullptr;     // [1 + N_z] work counter + per-plane arrival counters
+    int xy_occ = 0;
     bool zfft_attr_set = false;  // dynamic shared-memory limit of k_zfft_scale raised on this context's device
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;
@@ -276,6 +280,12 @@ bool zfft_supported(const pce_params& p);
 int zfft_init(pce_ctx* c);
 int zfft_scale(pce_ctx* c, const void* in, void* out, int deriv);  // deriv = -1: potential; 0..2: times -i k_d (field component d)
 
+// fftxy.cu
+bool fftxy_supported(const pce_params& p);
+int fftxy_init(pce_ctx* c);
+int fftxy_forward(pce_ctx* c, cufftDoubleComplex* gk);   // c->grid -> gk (x, y transformed, plane by plane)
+int fftxy_inverse(pce_ctx* c, cufftDoubleComplex* gk);   // gk -> c->grid
+
 // wave_bricks.cu
 int wave_bricks_init(pce_ctx* c);
 int wave_coef_alloc(pce_ctx* c, Bins& b);
@@ -294,6 +304,7 @@ int wave_gather_cols(pce_ctx* c, const Bins& b, bool field, double* psi_s, doubl
 
 // krylov.cu
 int bodies_setup(pce_ctx* c);
+int bodies_set_centres(pce_ctx* c, const double* X, const double* Y, const double* Z);
 int solve_cg(pce_ctx* c, const double* Q_body, const double* q_ion, const double E0[3], int warm, double* q, double* Phi, pce_solve_info* info);
 int solve_plain(pce_ctx* c, const double* b, double* q, pce_solve_info* info);  // M_bb q = b (no constraint), b and q device [Nbead]
 int capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_solve_info* info);

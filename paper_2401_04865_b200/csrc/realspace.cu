@@ -401,6 +401,16 @@ k_csr_rows(int n, CellGeom g, RealConst k, RealTable T, const int* __restrict__ 
     if (!FILL && lane == 0) row_ptr[i] = cnt;
 }
 
+// 64-bit total of the row counts (the int32 scan below would wrap silently past 2^31 entries)
+__global__ void __launch_bounds__(256) k_count_total(int n, const int* __restrict__ cnt, unsigned long long* __restrict__ total)
+{
+    unsigned long long v = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) v += (unsigned)cnt[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(total, v);
+}
+
 int real_csr_build(pce_ctx* c, const Bins& b)
 {
     c->nnz = 0;
@@ -417,12 +427,21 @@ int real_csr_build(pce_ctx* c, const Bins& b)
     else
         k_csr_count<<<cdiv(n, 128), 128, 0, c->st>>>(n, geom_of(b), c->rk.rc2, b.cell_start, b.xs, b.ys, b.zs, c->csr_ptr);
     c->launches++;
+    unsigned long long* total_d = reinterpret_cast<unsigned long long*>(c->scal + 32);
+    PCE_CUDA(c, cudaMemsetAsync(total_d, 0, sizeof(unsigned long long), c->st));
+    k_count_total<<<256, 256, 0, c->st>>>(n, c->csr_ptr, total_d);
+    c->launches++;
     int rc = exclusive_scan(c, c->csr_ptr, n + 1);
     if (rc) return rc;
     int nnz = 0;
+    unsigned long long total = 0;
     PCE_CUDA(c, cudaMemcpyAsync(&nnz, c->csr_ptr + n, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    PCE_CUDA(c, cudaMemcpyAsync(&total, total_d, sizeof(total), cudaMemcpyDeviceToHost, c->st));
     PCE_CUDA(c, cudaStreamSynchronize(c->st));
-    if (nnz < 0) { c->err = "near-field entry count overflows int32"; return PCE_ENOMEM; }
+    if (total > 0x7fffffffull || nnz < 0 || (unsigned long long)nnz != total) {
+        c->err = "near-field entry count overflows int32 (" + std::to_string(total) + " pairs within r_c)";
+        return PCE_ENOMEM;
+    }
     if (nnz > c->nnz_cap) {
         cudaFree(c->csr_col); cudaFree(c->csr_val);
         c->csr_col = nullptr; c->csr_val = nullptr;

@@ -65,6 +65,7 @@ k_scale(WaveConst wc, const cufftDoubleComplex* gin, cufftDoubleComplex* gout, i
 int wave_forward(pce_ctx* c)
 {
     PassTimer t(c, PASS_FFT);
+    if (c->use_fftxy) return fftxy_forward(c, c->gridk);
     if (cufftExecD2Z(c->planF, c->grid, c->gridk) != CUFFT_SUCCESS) { c->err = "cufftExecD2Z failed"; return PCE_ECUFFT; }
     return PCE_OK;
 }
@@ -95,6 +96,7 @@ int wave_scale_inverse(pce_ctx* c, int deriv)
     }
     {
         PassTimer t(c, PASS_IFFT);
+        if (c->use_fftxy) return fftxy_inverse(c, out);
         if (cufftExecZ2D(c->planB, out, c->grid) != CUFFT_SUCCESS) { c->err = "cufftExecZ2D failed"; return PCE_ECUFFT; }
     }
     return PCE_OK;

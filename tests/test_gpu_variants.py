@@ -107,3 +107,31 @@ def test_fiber_with_ions_full_parity():
     assert body_vector_error(out["F"].cpu().numpy(), oo["F"], oo["f"])[0] < 1e-8
     assert body_vector_error(out["T"].cpu().numpy(), oo["T"], oo["f"])[0] < 1e-8
     ctx.close()
+
+
+def test_set_centres_moves_the_reference_point_only():
+    """pce_set_centres (eq. 12): with X_i shifted by d_i the charges are unchanged, Phi_i grows by d_i.E0 (the
+    constant r.E0 loses), S_i = S_i - d_i Q_i and T_i = T_i - d_i x F_i -- textbook change of reference point, with the
+    un-shifted run already pinned to the oracle."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.tiny_random(seed=33, n_body=3, n_ion=30, L=7.0, Ng=32, neutral=True)
+    ctx = pce.context_for(w)
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    q0, Phi0, _ = ctx.solve(Q, qi, w.E0)
+    o0 = ctx.forces(q0, w.E0)
+    X0, _ = orc.body_centres(w.x, w.body_offset, w.L)
+    d = np.random.default_rng(1).normal(size=(w.N_body, 3)) * 0.3
+    Xn = torch.from_numpy(np.ascontiguousarray((X0 + d).T)).cuda()
+    ctx.set_centres(Xn[0].contiguous(), Xn[1].contiguous(), Xn[2].contiguous())
+    q1, Phi1, _ = ctx.solve(Q, qi, w.E0)
+    o1 = ctx.forces(q1, w.E0)
+    assert rel(q1.cpu().numpy(), q0.cpu().numpy()) < 1e-10
+    assert np.allclose(Phi1.cpu().numpy(), Phi0.cpu().numpy() + d @ w.E0, rtol=0, atol=1e-9 * np.abs(Phi0.cpu().numpy()).max())
+    F0, T0, S0 = (o0[k].cpu().numpy() for k in ("F", "T", "S"))
+    assert np.allclose(o1["F"].cpu().numpy(), F0, atol=1e-9 * np.abs(F0).max())
+    assert np.allclose(o1["S"].cpu().numpy(), S0 - d * w.Q_body[:, None], atol=1e-9 * np.abs(S0).max())
+    assert np.allclose(o1["T"].cpu().numpy(), T0 - np.cross(d, F0), atol=1e-9 * max(np.abs(T0).max(), np.abs(F0).max()))
+    ctx.close()
