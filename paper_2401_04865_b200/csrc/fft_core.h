@@ -3,6 +3,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cmath>
+#include <vector>
+
 namespace fftcore {
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -43,6 +46,49 @@ template <int R, int S> __device__ __forceinline__ void dftR(double2* v)
     else if (R == 4) dft4<S>(v);
     else dft2<S>(v);
 }
+
+// N = 8^n8 * rest (rest = 8 counts as one more radix-8 stage)
+template <int N> struct Radices {
+    static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;
+    static constexpr int n8 = (N == 16 || N == 32 || N == 64) ? (N == 64 ? 2 : 1) : (N == 128 || N == 256 || N == 512) ? (N == 512 ? 3 : 2) : 3;
+};
+
+
+// Twiddles: stage with Ns butterfly groups needs w_k^r, w_k = exp(S 2 pi i k / (Ns R)), k = b mod Ns.  They come from a compact
+// table per stage, tws[st] = [w_k | w_k^2 | w_k^4] (k < Ns, forward sign), so that the lanes of a warp read consecutive entries
+// (the full-length table indexed by k N / (Ns R) puts them a stride apart: bank conflicts); the rest are products.
+template <int R, int S>
+__device__ __forceinline__ void twiddle_dft_c(double2* v, const double2* __restrict__ t, int Ns, int k)
+{
+    if (Ns > 1) {
+        double2 w1 = t[k];
+        if (S > 0) w1.y = -w1.y;
+        if (R == 2) {
+            v[1] = cmul(v[1], w1);
+        } else {
+            double2 w2 = t[Ns + k];
+            if (S > 0) w2.y = -w2.y;
+            const double2 w3 = cmul(w1, w2);
+            v[1] = cmul(v[1], w1);
+            v[2] = cmul(v[2], w2);
+            v[3] = cmul(v[3], w3);
+            if (R == 8) {
+                double2 w4 = t[2 * Ns + k];
+                if (S > 0) w4.y = -w4.y;
+                v[4] = cmul(v[4], w4);
+                v[5] = cmul(v[5], cmul(w4, w1));
+                v[6] = cmul(v[6], cmul(w4, w2));
+                v[7] = cmul(v[7], cmul(w4, w3));
+            }
+        }
+    }
+    dftR<R, S>(v);
+}
+
+// offset of the table of the stage with Ns groups: stages Ns = 8, 64, 512 hold 3 Ns entries each
+__host__ __device__ constexpr int tw_offset(int Ns) { return Ns <= 8 ? 0 : Ns <= 64 ? 24 : Ns <= 512 ? 24 + 192 : 24 + 192 + 1536; }
+template <int N> struct TwSize { static constexpr int value = tw_offset(N / Radices<N>::rest) + 3 * (N / Radices<N>::rest); };
+
 
 // v[r] *= w^r, w = exp(S 2 pi i tstep / N) (table tw[m] = exp(-2 pi i m / N)), then the radix-R butterfly
 template <int R, int S>
@@ -99,7 +145,7 @@ __device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok
     for (int q = 0; q < NB; ++q) {
         const int b = j + q * NT;
         const int k = b & (Ns - 1);
-        twiddle_dft<R, S>(v + q * R, k * (N / (Ns * R)), tw);
+        twiddle_dft_c<R, S>(v + q * R, tw + tw_offset(Ns), Ns, k);
         const int d = (b - k) * R + k;
 #pragma unroll
         for (int r = 0; r < R; ++r)
@@ -108,10 +154,24 @@ __device__ __forceinline__ void stage(const double2* in, size_t istr, bool in_ok
 }
 
 
-// N = 8^n8 * rest (rest = 8 counts as one more radix-8 stage)
-template <int N> struct Radices {
-    static constexpr int rest = (N == 16 || N == 128 || N == 1024) ? 2 : (N == 32 || N == 256) ? 4 : 8;
-    static constexpr int n8 = (N == 16 || N == 32 || N == 64) ? (N == 64 ? 2 : 1) : (N == 128 || N == 256 || N == 512) ? (N == 512 ? 3 : 2) : 3;
-};
+
+// host: the per-stage tables of an n-point transform, n = 8^m * rest: stages Ns = 8, 64, ... of radix 8 but for the last one
+inline void stage_twiddles(int n, std::vector<double2>& tw)
+{
+    int rest = n;
+    while (rest > 8) rest /= 8;
+    const long double pi = 3.14159265358979323846264338327950288L;
+    tw.clear();
+    for (int Ns = 8; Ns < n; Ns *= 8) {
+        const int R = (Ns * 8 <= n) ? 8 : rest;
+        tw.resize(tw_offset(Ns));  // no-op by construction of tw_offset
+        for (int pw = 1; pw <= 4; pw *= 2)
+            for (int k = 0; k < Ns; ++k) {
+                const long double ang = -2.0L * pi * (long double)(pw * k) / (long double)(Ns * R);
+                tw.push_back(make_double2((double)cosl(ang), (double)sinl(ang)));
+            }
+    }
+    if (tw.empty()) tw.push_back(make_double2(1.0, 0.0));
+}
 
 }  // namespace fftcore

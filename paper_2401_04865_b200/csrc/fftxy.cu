@@ -18,14 +18,15 @@
 #include "pce_internal.h"
 #include "fft_core.h"
 
+#include <cstdlib>
+
 namespace {
 
 using namespace fftcore;
 
-constexpr int NT = 256;    // threads per CTA
-constexpr int DEPTH = 2;   // planes between the two passes of a plane
+constexpr int DEPTH = 8;   // planes between the two passes of a plane: more items than CTAs in flight, so that waits are rare
 
-template <int N> struct Geo {
+template <int N, int NT> struct Geo {
     static constexpr int TP = N / 8;          // threads per transform
     static constexpr int KP = NT / TP;        // transforms per CTA
     static constexpr int PS = N + N / 8 + (KP <= 2 ? 4 : KP <= 4 ? 2 : 1);  // pencil stride (elements)
@@ -34,42 +35,75 @@ template <int N> struct Geo {
 
 __device__ __forceinline__ int pad(int e) { return e + (e >> 3); }
 
-// one Stockham stage of radix R on the thread's 8 elements, in place in the padded pencil (barrier between loads and stores)
-template <int N, int R, int S>
-__device__ __forceinline__ void sstage(double2* pen, int Ns, int j, const double2* __restrict__ tw)
+// Pieces of one Stockham stage of radix R on the thread's 8 elements (8 / R butterflies): butterfly q is b = j + q N/8,
+// its inputs are the elements b + r N/R, its outputs go to (b - k) R + k + r Ns with k = b mod Ns.
+template <int N, int R>
+__device__ __forceinline__ int in_index(int j, int q, int r) { return j + q * (N / 8) + r * (N / R); }
+template <int N, int R>
+__device__ __forceinline__ int out_index(int Ns, int j, int q, int r)
 {
-    constexpr int NB = 8 / R, TP = N / 8;
-    double2 v[8];
+    const int b = j + q * (N / 8), k = b & (Ns - 1);
+    return (b - k) * R + k + r * Ns;
+}
+template <int N, int R, int S>
+__device__ __forceinline__ void compute_stage(double2* v, int Ns, int j, const double2* __restrict__ tw)
+{
 #pragma unroll
-    for (int q = 0; q < NB; ++q) {
-        const int b = j + q * TP;
-#pragma unroll
-        for (int r = 0; r < R; ++r) v[q * R + r] = pen[pad(b + r * (N / R))];
+    for (int q = 0; q < 8 / R; ++q) {
+        const int b = j + q * (N / 8);
+        twiddle_dft_c<R, S>(v + q * R, tw + tw_offset(Ns), Ns, b & (Ns - 1));
     }
-    __syncthreads();
+}
+template <int N, int R>
+__device__ __forceinline__ void load_stage(const double2* pen, int j, double2* v)
+{
 #pragma unroll
-    for (int q = 0; q < NB; ++q) {
-        const int b = j + q * TP;
-        const int k = b & (Ns - 1);
-        twiddle_dft<R, S>(v + q * R, k * (N / (Ns * R)), tw);
-        const int d = (b - k) * R + k;
+    for (int q = 0; q < 8 / R; ++q)
 #pragma unroll
-        for (int r = 0; r < R; ++r) pen[pad(d + r * Ns)] = v[q * R + r];
-    }
-    __syncthreads();
+        for (int r = 0; r < R; ++r) v[q * R + r] = pen[pad(in_index<N, R>(j, q, r))];
+}
+template <int N, int R>
+__device__ __forceinline__ void store_stage(double2* pen, int Ns, int j, const double2* v)
+{
+#pragma unroll
+    for (int q = 0; q < 8 / R; ++q)
+#pragma unroll
+        for (int r = 0; r < R; ++r) pen[pad(out_index<N, R>(Ns, j, q, r))] = v[q * R + r];
 }
 
-// N-point transform of the pencil (natural order in and out); the data must be in place and visible (barrier before the call)
-template <int N, int S>
-__device__ __forceinline__ void fft_smem(double2* pen, int j, const double2* __restrict__ tw)
+// barrier over the threads that share a pencil: the whole CTA (WHOLE: a warp touches every pencil) or the N/8 threads of the
+// transform (consecutive threads: named barrier 1 + p for two or more warps, else the warp)
+template <int N, bool WHOLE>
+__device__ __forceinline__ void pencil_sync(int p)
+{
+    if (WHOLE) __syncthreads();
+    else if (N / 8 >= 64) asm volatile("bar.sync %0, %1;" ::"r"(1 + p), "r"(N / 8) : "memory");
+    else __syncwarp();
+}
+
+// The transform with its first stage fed from registers and its last stage left in registers:
+//   in:  v[r] = element j + r N/8 (the inputs of the first radix-8 stage);  out: v[q R + r] = element out_index<N, REST>(N/REST, j, q, r)
+// (natural order).  The pencil is scratch; barriers as pencil_sync<N, WHOLE>.
+template <int N, int S, bool WHOLE>
+__device__ __forceinline__ void fft_regs(double2* v, double2* pen, int p, int j, const double2* __restrict__ tw)
 {
     constexpr int REST = Radices<N>::rest, N8 = Radices<N>::n8;
-    constexpr int NF8 = (REST == 8) ? N8 - 1 : N8;
-    int Ns = 1;
-    if (NF8 >= 1) { sstage<N, 8, S>(pen, Ns, j, tw); Ns *= 8; }
-    if (NF8 >= 2) { sstage<N, 8, S>(pen, Ns, j, tw); Ns *= 8; }
-    if (NF8 >= 3) { sstage<N, 8, S>(pen, Ns, j, tw); Ns *= 8; }
-    sstage<N, REST, S>(pen, Ns, j, tw);
+    constexpr int NF8 = (REST == 8) ? N8 - 1 : N8;   // radix-8 stages before the last stage (radix REST)
+    compute_stage<N, 8, S>(v, 1, j, tw);
+    store_stage<N, 8>(pen, 1, j, v);
+    pencil_sync<N, WHOLE>(p);
+    int Ns = 8;
+#pragma unroll
+    for (int st = 1; st < NF8; ++st) {
+        load_stage<N, 8>(pen, j, v);
+        pencil_sync<N, WHOLE>(p);
+        compute_stage<N, 8, S>(v, Ns, j, tw);
+        store_stage<N, 8>(pen, Ns, j, v);
+        pencil_sync<N, WHOLE>(p);
+        Ns *= 8;
+    }
+    load_stage<N, REST>(pen, j, v);
+    compute_stage<N, REST, S>(v, Ns, j, tw);
 }
 
 // item id -> (kind, plane, index): slot s holds the n1 first-pass items of plane s (s < nz) and then the n2 second-pass items
@@ -102,104 +136,121 @@ __device__ __forceinline__ void signal_plane(int* done)
     if (threadIdx.x == 0) atomicAdd(done, 1);
 }
 
-// columns kx0 .. kx0+KP-1 of plane z: N-point transforms along y, in place in the half spectrum
-template <int N, int S>
+// columns kx0 .. kx0+KP-1 of plane z: N-point transforms along y, in place in the half spectrum.  Thread (j, p), p fastest: a
+// warp reads KP consecutive columns (KP x 16 bytes contiguous) of 32 / KP rows; first stage from global memory, last stage to it.
+template <int N, int NT, int S>
 __device__ __forceinline__ void y_item(double2* gk, int nxh, int z, int b, double2* tile, const double2* __restrict__ tw)
 {
-    using G = Geo<N>;
+    using G = Geo<N, NT>;
+    constexpr int REST = Radices<N>::rest;
     const int p = threadIdx.x % G::KP, j = threadIdx.x / G::KP;
     const int kx = b * G::KP + p;
     const bool ok = kx < nxh;
     double2* col = gk + (size_t)z * N * nxh + (ok ? kx : 0);
-    double2* pen = tile + p * G::PS;
+    double2 v[8];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-        const int y = j + r * G::TP;
-        pen[pad(y)] = ok ? __ldcg(col + (size_t)y * nxh) : make_double2(0.0, 0.0);
-    }
-    __syncthreads();
-    fft_smem<N, S>(pen, j, tw);
+    for (int r = 0; r < 8; ++r) v[r] = __ldcg(col + (size_t)(j + r * G::TP) * nxh);
+    fft_regs<N, S, true>(v, tile + p * G::PS, p, j, tw);
     if (ok) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int y = j + r * G::TP;
-            col[(size_t)y * nxh] = pen[pad(y)];
-        }
+        for (int q = 0; q < 8 / REST; ++q)
+#pragma unroll
+            for (int r = 0; r < REST; ++r) col[(size_t)out_index<N, REST>(N / REST, j, q, r) * nxh] = v[q * REST + r];
     }
-    __syncthreads();
 }
 
-// rows 2 KP a .. 2 KP a + 2 KP - 1 of plane z: real -> half-complex along x (two rows per transform)
-template <int N>
+// rows 2 KP a .. 2 KP a + 2 KP - 1 of plane z: real -> half-complex along x, two rows per transform.  Thread (p, j), j fastest:
+// the N/8 threads of a transform are consecutive, read their two rows coalesced, and synchronise among themselves only.
+template <int N, int NT>
 __device__ __forceinline__ void x_item_fwd(const double* __restrict__ grid, double2* gk, int nxh, int z, int a, double2* tile,
                                            const double2* __restrict__ tw)
 {
-    using G = Geo<N>;
-    const size_t row0 = (size_t)z * N + (size_t)a * 2 * G::KP;
-    for (int i = threadIdx.x; i < G::KP * N; i += NT) {  // consecutive lanes: consecutive x of one row pair
-        const int pp = i / N, e = i % N;
-        const double* ra = grid + (row0 + 2 * pp) * N;
-        tile[pp * G::PS + pad(e)] = make_double2(__ldg(ra + e), __ldg(ra + N + e));
+    using G = Geo<N, NT>;
+    constexpr int REST = Radices<N>::rest;
+    const int p = threadIdx.x / G::TP, j = threadIdx.x % G::TP;
+    const size_t row = (size_t)z * N + (size_t)a * 2 * G::KP + 2 * p;
+    const double* ra = grid + row * N;
+    double2* pen = tile + p * G::PS;
+    double2 v[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) v[r] = make_double2(__ldg(ra + j + r * G::TP), __ldg(ra + N + j + r * G::TP));
+    fft_regs<N, -1, false>(v, pen, p, j, tw);
+    pencil_sync<N, false>(p);   // every thread has read its last-stage inputs: the pencil can take the spectrum
+#pragma unroll
+    for (int q = 0; q < 8 / REST; ++q)
+#pragma unroll
+        for (int r = 0; r < REST; ++r) pen[pad(out_index<N, REST>(N / REST, j, q, r))] = v[q * REST + r];
+    pencil_sync<N, false>(p);
+    double2* oa = gk + row * nxh;
+    for (int k = j; k <= N / 2; k += G::TP) {
+        const double2 Z = pen[pad(k)], Zc = pen[pad((N - k) & (N - 1))];
+        oa[k] = make_double2(0.5 * (Z.x + Zc.x), 0.5 * (Z.y - Zc.y));            // X_a = (Z(k) + conj Z(N-k)) / 2
+        oa[nxh + k] = make_double2(0.5 * (Z.y + Zc.y), -0.5 * (Z.x - Zc.x));     // X_b = (Z(k) - conj Z(N-k)) / (2i)
     }
-    __syncthreads();
-    fft_smem<N, -1>(tile + (threadIdx.x % G::KP) * G::PS, threadIdx.x / G::KP, tw);
-    for (int i = threadIdx.x; i < G::KP * G::NH; i += NT) {
-        const int pp = i / G::NH, k = i % G::NH;
-        const double2 Z = tile[pp * G::PS + pad(k)], Zc = tile[pp * G::PS + pad((N - k) & (N - 1))];
-        double2* oa = gk + (row0 + 2 * pp) * nxh + k;
-        oa[0] = make_double2(0.5 * (Z.x + Zc.x), 0.5 * (Z.y - Zc.y));      // X_a = (Z(k) + conj Z(N-k)) / 2
-        oa[nxh] = make_double2(0.5 * (Z.y + Zc.y), -0.5 * (Z.x - Zc.x));   // X_b = (Z(k) - conj Z(N-k)) / (2i)
-    }
-    __syncthreads();
 }
 
 // the reverse: half-complex rows -> two real rows per transform (unnormalised, as cuFFT's Z2D)
-template <int N>
+template <int N, int NT>
 __device__ __forceinline__ void x_item_inv(const double2* gk, double* __restrict__ grid, int nxh, int z, int a, double2* tile,
                                            const double2* __restrict__ tw)
 {
-    using G = Geo<N>;
-    const size_t row0 = (size_t)z * N + (size_t)a * 2 * G::KP;
-    for (int i = threadIdx.x; i < G::KP * G::NH; i += NT) {
-        const int pp = i / G::NH, k = i % G::NH;
-        const double2* ia = gk + (row0 + 2 * pp) * nxh + k;
-        double2 A = __ldcg(ia), B = __ldcg(ia + nxh);
+    using G = Geo<N, NT>;
+    constexpr int REST = Radices<N>::rest;
+    const int p = threadIdx.x / G::TP, j = threadIdx.x % G::TP;
+    const size_t row = (size_t)z * N + (size_t)a * 2 * G::KP + 2 * p;
+    const double2* ia = gk + row * nxh;
+    double2* pen = tile + p * G::PS;
+    for (int k = j; k <= N / 2; k += G::TP) {
+        double2 A = __ldcg(ia + k), B = __ldcg(ia + nxh + k);
         if (k == 0 || k == N / 2) { A.y = 0.0; B.y = 0.0; }  // the imaginary parts of the self-conjugate modes carry no information
-        double2* pen = tile + pp * G::PS;
-        pen[pad(k)] = make_double2(A.x - B.y, A.y + B.x);                          // Z(k) = X_a + i X_b
+        pen[pad(k)] = make_double2(A.x - B.y, A.y + B.x);                              // Z(k) = X_a + i X_b
         if (k > 0 && k < N / 2) pen[pad(N - k)] = make_double2(A.x + B.y, B.x - A.y);  // Z(N-k) = conj X_a + i conj X_b
     }
-    __syncthreads();
-    fft_smem<N, +1>(tile + (threadIdx.x % G::KP) * G::PS, threadIdx.x / G::KP, tw);
-    for (int i = threadIdx.x; i < G::KP * N; i += NT) {
-        const int pp = i / N, e = i % N;
-        const double2 v = tile[pp * G::PS + pad(e)];
-        double* ra = grid + (row0 + 2 * pp) * N;
-        ra[e] = v.x;
-        ra[N + e] = v.y;
-    }
-    __syncthreads();
+    pencil_sync<N, false>(p);
+    double2 v[8];
+    load_stage<N, 8>(pen, j, v);
+    pencil_sync<N, false>(p);
+    fft_regs<N, +1, false>(v, pen, p, j, tw);
+    double* ra = grid + row * N;
+#pragma unroll
+    for (int q = 0; q < 8 / REST; ++q)
+#pragma unroll
+        for (int r = 0; r < REST; ++r) {
+            const int e = out_index<N, REST>(N / REST, j, q, r);
+            ra[e] = v[q * REST + r].x;
+            ra[N + e] = v[q * REST + r].y;
+        }
 }
 
 // ctr[0]: work counter; ctr[1 + z]: arrivals of the first pass of plane z (both zeroed before the launch)
-template <int N, bool INVERSE>
-__global__ void __launch_bounds__(NT, 3)
+template <int N, int NT, bool INVERSE>
+__global__ void __launch_bounds__(NT, 1024 / NT)
 k_fft_xy(const double* gin, double* gout, double2* gk, int nz, const double2* __restrict__ tw_g, int* __restrict__ ctr,
          const int* __restrict__ skip)
 {
     if (skip && *skip) return;
-    using G = Geo<N>;
+    using G = Geo<N, NT>;
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* tile = reinterpret_cast<double2*>(fsm);   // [KP][PS]
-    double2* tw = tile + G::KP * G::PS;                // [N]
+    double2* tw = tile + G::KP * G::PS;                // per-stage twiddle tables
     __shared__ int s_item;
-    for (int i = threadIdx.x; i < N; i += NT) tw[i] = tw_g[i];
+    for (int i = threadIdx.x; i < TwSize<N>::value; i += NT) tw[i] = tw_g[i];
     constexpr int nxh = G::NH;
     constexpr int nX = N / (2 * G::KP), nY = (nxh + G::KP - 1) / G::KP;
     constexpr int n1 = INVERSE ? nY : nX, n2 = INVERSE ? nX : nY;
     const int total = nz * (n1 + n2);
+    // inverse: the rows an x item has consumed are dead (as with cuFFT's Z2D the spectrum does not survive); telling L2 so saves
+    // their write-back -- the y pass left them dirty in L2 and they never need to reach HBM
+    constexpr size_t blk_bytes = (size_t)2 * G::KP * nxh * sizeof(double2);
+    constexpr bool can_discard = INVERSE && (blk_bytes % 128 == 0);
+    unsigned char* dead = nullptr;
     for (;;) {
         __syncthreads();
+        if (can_discard && dead) {
+            for (size_t o = (size_t)threadIdx.x * 128; o < blk_bytes; o += (size_t)NT * 128)
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(dead + o) : "memory");
+            dead = nullptr;
+        }
         if (threadIdx.x == 0) s_item = atomicAdd(&ctr[0], 1);
         __syncthreads();
         const int id = s_item;
@@ -207,47 +258,49 @@ k_fft_xy(const double* gin, double* gout, double2* gk, int nz, const double2* __
         int second, z, idx;
         decode_item(id, nz, n1, n2, second, z, idx);
         if (!second) {
-            if (INVERSE) y_item<N, +1>(gk, nxh, z, idx, tile, tw);
-            else x_item_fwd<N>(gin, gk, nxh, z, idx, tile, tw);
+            if (INVERSE) y_item<N, NT, +1>(gk, nxh, z, idx, tile, tw);
+            else x_item_fwd<N, NT>(gin, gk, nxh, z, idx, tile, tw);
             signal_plane(&ctr[1 + z]);
         } else {
             wait_plane(&ctr[1 + z], n1);
-            if (INVERSE) x_item_inv<N>(gk, gout, nxh, z, idx, tile, tw);
-            else y_item<N, -1>(gk, nxh, z, idx, tile, tw);
+            if (INVERSE) {
+                x_item_inv<N, NT>(gk, gout, nxh, z, idx, tile, tw);
+                dead = reinterpret_cast<unsigned char*>(gk + ((size_t)z * N + (size_t)idx * 2 * G::KP) * nxh);
+            }
+            else y_item<N, NT, -1>(gk, nxh, z, idx, tile, tw);
         }
     }
 }
 
-template <int N> size_t smem_of() { return (size_t)(Geo<N>::KP * Geo<N>::PS + N) * sizeof(double2); }
+template <int N, int NT> size_t smem_of() { return (size_t)(Geo<N, NT>::KP * Geo<N, NT>::PS + TwSize<N>::value) * sizeof(double2); }
 
-template <int N> int launch_xy(pce_ctx* c, bool inverse, cufftDoubleComplex* gk)
+template <int N, int NT, bool INVERSE> int launch_one(pce_ctx* c, cufftDoubleComplex* gk)
 {
-    const size_t smem = smem_of<N>();
+    using G = Geo<N, NT>;
+    const size_t smem = smem_of<N, NT>();
     const int nz = c->wk.Ng[2];
+    int& occ = c->xy_occ[INVERSE ? 1 : 0];
+    if (occ == 0) {  // first use on this context: raise the shared-memory limit, size the persistent grid
+        PCE_CUDA(c, cudaFuncSetAttribute(k_fft_xy<N, NT, INVERSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fft_xy<N, NT, INVERSE>, NT, smem));
+        if (occ < 1) { c->err = "fftxy kernels do not fit on this device"; return PCE_ECUDA; }
+    }
     PCE_CUDA(c, cudaMemsetAsync(c->xy_ctr, 0, ((size_t)nz + 1) * sizeof(int), c->st));
-    const int total = nz * (N / (2 * Geo<N>::KP) + (Geo<N>::NH + Geo<N>::KP - 1) / Geo<N>::KP);
-    int blocks = c->num_sm * c->xy_occ;
+    const int total = nz * (N / (2 * G::KP) + (G::NH + G::KP - 1) / G::KP);
+    int blocks = c->num_sm * occ;
     if (blocks > total) blocks = total;
-    if (inverse)
-        k_fft_xy<N, true><<<blocks, NT, smem, c->st>>>(nullptr, c->grid, reinterpret_cast<double2*>(gk), nz, c->xytw, c->xy_ctr, c->skip_flag);
-    else
-        k_fft_xy<N, false><<<blocks, NT, smem, c->st>>>(c->grid, nullptr, reinterpret_cast<double2*>(gk), nz, c->xytw, c->xy_ctr, c->skip_flag);
+    k_fft_xy<N, NT, INVERSE><<<blocks, NT, smem, c->st>>>(INVERSE ? nullptr : c->grid, INVERSE ? c->grid : nullptr, reinterpret_cast<double2*>(gk),
+                                                         nz, c->xytw, c->xy_ctr, c->skip_flag);
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
 }
 
-template <int N> int init_xy(pce_ctx* c)
+template <int N, bool INVERSE> int launch_xy(pce_ctx* c, cufftDoubleComplex* gk)
 {
-    const int smem = (int)smem_of<N>();
-    PCE_CUDA(c, cudaFuncSetAttribute(k_fft_xy<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    PCE_CUDA(c, cudaFuncSetAttribute(k_fft_xy<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    int o1 = 0, o2 = 0;
-    PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o1, k_fft_xy<N, true>, NT, smem));
-    PCE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o2, k_fft_xy<N, false>, NT, smem));
-    c->xy_occ = o1 < o2 ? o1 : o2;
-    if (c->xy_occ < 1) { c->err = "fftxy kernels do not fit on this device"; return PCE_ECUDA; }
-    return PCE_OK;
+    if (c->xy_nt[INVERSE ? 1 : 0] == 128) return launch_one<N, 128, INVERSE>(c, gk);
+    if (c->xy_nt[INVERSE ? 1 : 0] == 512) return launch_one<N, 512, INVERSE>(c, gk);
+    return launch_one<N, 256, INVERSE>(c, gk);
 }
 
 }  // namespace
@@ -264,36 +317,35 @@ bool fftxy_supported(const pce_params& p)
 int fftxy_init(pce_ctx* c)
 {
     const int n = c->p.Ng[0];
-    std::vector<double2> tw(n);
-    const long double pi = 3.14159265358979323846264338327950288L;
-    for (int m = 0; m < n; ++m) tw[m] = make_double2((double)cosl(-2.0L * pi * m / n), (double)sinl(-2.0L * pi * m / n));
-    PCE_CUDA(c, cudaMalloc(&c->xytw, n * sizeof(double2)));
-    PCE_CUDA(c, cudaMemcpy(c->xytw, tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice));
+    std::vector<double2> tw;
+    stage_twiddles(n, tw);
+    PCE_CUDA(c, cudaMalloc(&c->xytw, tw.size() * sizeof(double2)));
+    PCE_CUDA(c, cudaMemcpy(c->xytw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice));
     PCE_CUDA(c, cudaMalloc(&c->xy_ctr, ((size_t)c->p.Ng[2] + 1) * sizeof(int)));
-    switch (n) {
-        case 128: return init_xy<128>(c);
-        case 256: return init_xy<256>(c);
-        case 512: return init_xy<512>(c);
-        default: return init_xy<1024>(c);
-    }
+    const char* ef = getenv("PCE_FFTXY_NT_F");
+    const char* ei = getenv("PCE_FFTXY_NT_I");
+    c->xy_nt[0] = (ef && (atoi(ef) == 128 || atoi(ef) == 512)) ? atoi(ef) : 256;
+    c->xy_nt[1] = (ei && (atoi(ei) == 128 || atoi(ei) == 512)) ? atoi(ei) : 256;
+    c->xy_occ[0] = c->xy_occ[1] = 0;
+    return PCE_OK;
 }
 
 int fftxy_forward(pce_ctx* c, cufftDoubleComplex* gk)
 {
     switch (c->p.Ng[0]) {
-        case 128: return launch_xy<128>(c, false, gk);
-        case 256: return launch_xy<256>(c, false, gk);
-        case 512: return launch_xy<512>(c, false, gk);
-        default: return launch_xy<1024>(c, false, gk);
+        case 128: return launch_xy<128, false>(c, gk);
+        case 256: return launch_xy<256, false>(c, gk);
+        case 512: return launch_xy<512, false>(c, gk);
+        default: return launch_xy<1024, false>(c, gk);
     }
 }
 
 int fftxy_inverse(pce_ctx* c, cufftDoubleComplex* gk)
 {
     switch (c->p.Ng[0]) {
-        case 128: return launch_xy<128>(c, true, gk);
-        case 256: return launch_xy<256>(c, true, gk);
-        case 512: return launch_xy<512>(c, true, gk);
-        default: return launch_xy<1024>(c, true, gk);
+        case 128: return launch_xy<128, true>(c, gk);
+        case 256: return launch_xy<256, true>(c, gk);
+        case 512: return launch_xy<512, true>(c, gk);
+        default: return launch_xy<1024, true>(c, gk);
     }
 }

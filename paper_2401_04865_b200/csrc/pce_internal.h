@@ -153,7 +153,7 @@ struct pce_ctx {
     bool use_fftxy = false;    // own (x, y) transforms, one HBM trip per plane and direction (fftxy.cu) instead of cuFFT 2-D plans
     double2* xytw = nullptr;   // twiddles exp(-2 pi i m / N_x)
     int* xy_ctr = nullptr;     // [1 + N_z] work counter + per-plane arrival counters
-    int xy_occ = 0;
+    int xy_occ[2] = {0, 0}, xy_nt[2] = {128, 128};  // per direction (forward, inverse): resident CTAs per SM, threads per CTA
     bool zfft_attr_set = false;  // dynamic shared-memory limit of k_zfft_scale raised on this context's device
     // persistent brick kernels (wave_bricks.cu)
     int num_sm = 0, occ_spread = 0, occ_gather = 0, occ_gather_f = 0;

@@ -64,7 +64,7 @@ __device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const do
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const int b = j + q * NTH;  // b < N / R = Ns: k = b, twiddle step k N / (Ns R) = b
-        twiddle_dft<R, -1>(v + q * R, b, tw);
+        twiddle_dft_c<R, -1>(v + q * R, tw + tw_offset(N / R), N / R, b);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int iz = b + r * (N / R);
@@ -75,10 +75,17 @@ __device__ __forceinline__ void fused_middle(double2* sp, int j, int p, const do
                 v[q * R + r] = make_double2(v[q * R + r].y * kd, -v[q * R + r].x * kd);
             }
         }
-        dftR<R, +1>(v + q * R);  // Ns = 1: no twiddles; outputs at b R + r
-#pragma unroll
-        for (int r = 0; r < R; ++r) sp[(size_t)(b * R + r) * KP] = v[q * R + r];
     }
+    // first inverse stage, radix 8 (the same stage order as the forward transform, so both share the twiddle tables): the
+    // thread holds the elements j + m N/8, slot (q, r) of the radix-R stage being m = q + r 8/R
+    double2 w[8];
+#pragma unroll
+    for (int q = 0; q < NB; ++q)
+#pragma unroll
+        for (int r = 0; r < R; ++r) w[q + r * NB] = v[q * R + r];
+    dft8<+1>(w);  // Ns = 1: no twiddles; outputs at 8 j + r
+#pragma unroll
+    for (int r = 0; r < 8; ++r) sp[(size_t)(8 * j + r) * KP] = w[r];
 }
 template <int N>
 __global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 3 : 1)
@@ -88,11 +95,11 @@ k_zfft_scale(WaveConst wc, const double2* gin, double2* gout, int deriv, const d
     if (skip && *skip) return;
     extern __shared__ __align__(16) unsigned char zsm[];
     double2* tile = reinterpret_cast<double2*>(zsm);       // [N][KP]
-    double2* tw = tile + (size_t)N * KP;                    // [N]
-    double* gs = reinterpret_cast<double*>(tw + N);         // [N][KP] Green's function of the CTA's pencils
+    double2* tw = tile + (size_t)N * KP;                    // per-stage twiddle tables (fft_core.h)
+    double* gs = reinterpret_cast<double*>(tw + TwSize<N>::value);  // [N][KP] Green's function of the CTA's pencils
     constexpr int REST = Radices<N>::rest, N8 = Radices<N>::n8;
     const int tid = threadIdx.x, p = tid % KP, j = tid / KP;
-    for (int i = tid; i < N; i += N / 8 * KP) tw[i] = tw_g[i];
+    for (int i = tid; i < TwSize<N>::value; i += N / 8 * KP) tw[i] = tw_g[i];
     const int nxh = wc.Nxh, ny = wc.Ng[1];
     const int kxi = blockIdx.x * KP + p, iy = blockIdx.y;  // iy in [0, ny/2]
     const bool col_ok = kxi < nxh;
@@ -137,142 +144,17 @@ k_zfft_scale(WaveConst wc, const double2* gin, double2* gout, int deriv, const d
         // registers: the forward stage leaves element b + r N/REST in slot r, which is what the inverse stage reads
         fused_middle<N, REST>(sp, j, p, tw, gs, deriv, kxy, wc.kfac[2]);
         __syncthreads();
-        // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
-        Ns = REST;
-        if (NF8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
+        // ---- inverse: the remaining radix-8 stages, then the stage of radix REST straight to global memory
+        Ns = 8;
         if (NF8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
-    }
-}
-
-// ---------------------------------------------------------------- pipelined variant (N_z = 64 ... 1024 with N = 8^m * rest)
-// Same arithmetic, arranged so that HBM is kept busy: persistent CTAs walk (k_x tile, |k_y|) pairs; the [N_z][KP] tile of the
-// NEXT row streams into a second shared-memory buffer with cp.async while the current row runs its stages; the last forward
-// stage, the multiplication by the Green's function and the first inverse stage are one register-resident step (the last
-// forward stage of radix R leaves element b + r N/R in slot r, which is exactly what the first inverse stage of radix R reads),
-// so a row costs 2 fewer shared-memory passes and 3 fewer barriers.
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem_src) : "memory");
-}
-
-template <int N>
-__global__ void __launch_bounds__(N / 8 * KP, (N <= 512) ? 2 : 1)
-k_zfft_scale_pipe(WaveConst wc, double2* __restrict__ gk, const double2* __restrict__ tw_g, const double* __restrict__ zexp,
-                  const double* __restrict__ shape, int shape_key_lo, const int* __restrict__ skip)
-{
-    if (skip && *skip) return;
-    constexpr int REST = Radices<N>::rest, N8 = Radices<N>::n8;   // N = 8^N8 * REST (REST = 8 counts as one more radix-8 stage)
-    constexpr int NT = N / 8 * KP;
-    extern __shared__ __align__(16) unsigned char zsm[];
-    double2* tile0 = reinterpret_cast<double2*>(zsm);        // [2][N][KP]
-    double2* tw = tile0 + (size_t)2 * N * KP;                 // [N]
-    double* gs = reinterpret_cast<double*>(tw + N);           // [N][KP]
-    const int tid = threadIdx.x, p = tid % KP, j = tid / KP;
-    for (int i = tid; i < N; i += NT) tw[i] = tw_g[i];
-    const int nxh = wc.Nxh, ny = wc.Ng[1];
-    const int ntx = (nxh + KP - 1) / KP, nyh = ny / 2 + 1;
-    const int npairs = ntx * nyh;
-    const size_t zstr = (size_t)ny * nxh;
-    // rows of this CTA, flattened: pair = blockIdx.x + m gridDim.x, pass 0 (row iy) and, unless self-mirrored, pass 1 (row ny - iy)
-    auto row_of = [&](int pair, int pass, int& y, int& tx) {
-        tx = pair % ntx;
-        const int iy = pair / ntx;
-        y = (pass == 0) ? iy : ((iy == 0 || 2 * iy == ny) ? -1 : ny - iy);
-    };
-    auto issue = [&](int pair, int pass, double2* buf) {  // cp.async of one row tile; columns beyond N_x/2 re-read the last one
-        int y, tx;
-        row_of(pair, pass, y, tx);
-        const int kx = min(tx * KP + p, nxh - 1);
-        const double2* col = gk + (size_t)y * nxh + kx;
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int z = j + r * (N / 8);
-            cp_async16(buf + z * KP + p, col + (size_t)z * zstr);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
-    int pair = blockIdx.x, pass = 0, cur = 0;
-    if (pair >= npairs) return;
-    issue(pair, 0, tile0);
-    while (pair < npairs) {
-        // the row after this one
-        int npair = pair, npass = pass + 1;
-        {
-            int y1, tx1;
-            if (npass == 1) row_of(pair, 1, y1, tx1);
-            if (npass == 2 || y1 < 0) { npair = pair + gridDim.x; npass = 0; }
-        }
-        double2* sp_tile = tile0 + (size_t)cur * N * KP;
-        __syncthreads();  // the other buffer (previous row) and the Green's function table are free again
-        if (npair < npairs) issue(npair, npass, tile0 + (size_t)(cur ^ 1) * N * KP);
-        int y, tx;
-        row_of(pair, pass, y, tx);
-        if (pass == 0) {  // Green's function of the pair (even in k_y and k_z): N/2 + 1 evaluations per pencil
-            const int iy = pair / ntx;
-            const double ky = wc.kfac[1] * iy;
-            const double* ez = zexp + nxh + ny / 2 + 1;
-            for (int e = tid; e < (N / 2 + 1) * KP; e += NT) {
-                const int iz = e / KP, pp = e % KP, kxe = tx * KP + pp;
-                double f = 0.0;  // k = 0 removed; pencils beyond N_x/2 unused
-                if (kxe < nxh) {
-                    const double kx = wc.kfac[0] * kxe, kz = wc.kfac[2] * (double)iz;
-                    const double k2 = kx * kx + ky * ky + kz * kz;
-                    if (k2 > 0.0) f = wc.scale_norm * zexp[kxe] * zexp[nxh + iy] * ez[iz] * shape_eval(shape, shape_key_lo, k2);
-                }
-                gs[iz * KP + pp] = f;
-                if (iz > 0 && iz < N / 2) gs[(N - iz) * KP + pp] = f;
-            }
-        }
-        if (npair < npairs) asm volatile("cp.async.wait_group 1;" ::: "memory");
-        else asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncthreads();
-        const int kxi = tx * KP + p;
-        const bool col_ok = kxi < nxh;
-        double2* col = gk + (size_t)y * nxh + (col_ok ? kxi : 0);
-        double2* sp = sp_tile + p;
-        // ---- forward: all radix-8 stages but the last stage of the transform, in place
-        int Ns = 1;
-        constexpr int NF8 = (REST == 8) ? N8 - 1 : N8;  // radix-8 stages before the fused one
-        if (NF8 >= 1) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        if (NF8 >= 2) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        if (NF8 >= 3) { stage<N, 8, -1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        // ---- last forward stage x Green's function x first inverse stage, in registers
-        fused_middle<N, REST>(sp, j, p, tw, gs, -1, 0.0, 0.0);
-        __syncthreads();
-        // ---- inverse: the remaining radix-8 stages, the last one straight to global memory
-        Ns = REST;
         if (NF8 >= 3) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        if (NF8 >= 2) { stage<N, 8, +1, true>(sp, KP, true, sp, KP, true, Ns, j, tw, nullptr); __syncthreads(); Ns *= 8; }
-        stage<N, 8, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
-        pair = npair; pass = npass; cur ^= 1;
+        stage<N, REST, +1, false>(sp, KP, true, col, zstr, col_ok, Ns, j, tw, nullptr);
     }
-}
-
-template <int N> int launch_pipe(pce_ctx* c)
-{
-    const size_t smem = (size_t)2 * N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
-    if (!c->zfft_attr_set) {
-        PCE_CUDA(c, cudaFuncSetAttribute(k_zfft_scale_pipe<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        c->zfft_attr_set = true;
-    }
-    const int npairs = cdiv(c->wk.Nxh, KP) * (c->wk.Ng[1] / 2 + 1);
-    int per_sm = (int)((220 * 1024) / (smem + 1024));
-    if (per_sm > 2) per_sm = 2;
-    if (per_sm < 1) per_sm = 1;
-    int blocks = c->num_sm * per_sm;
-    if (blocks > npairs) blocks = npairs;
-    k_zfft_scale_pipe<N><<<blocks, N / 8 * KP, smem, c->st>>>(c->wk, reinterpret_cast<double2*>(c->gridk), c->ztw, c->zexp, c->zshape,
-                                                             c->zshape_key_lo, c->skip_flag);
-    c->launches++;
-    PCE_CUDA(c, cudaGetLastError());
-    return PCE_OK;
 }
 
 template <int N> int launch(pce_ctx* c, const double2* gin, double2* gout, int deriv)
 {
-    const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)N * sizeof(double2) + (size_t)N * KP * sizeof(double);
+    const size_t smem = (size_t)N * KP * sizeof(double2) + (size_t)TwSize<N>::value * sizeof(double2) + (size_t)N * KP * sizeof(double);
     if (!c->zfft_attr_set && smem > 48 * 1024) {  // the attribute is per device: once per context, not per process
         PCE_CUDA(c, cudaFuncSetAttribute(k_zfft_scale<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->zfft_attr_set = true;
@@ -296,11 +178,10 @@ bool zfft_supported(const pce_params& p)
 int zfft_init(pce_ctx* c)
 {
     const int n = c->p.Ng[2];
-    std::vector<double2> tw(n);
-    const long double pi = 3.14159265358979323846264338327950288L;
-    for (int m = 0; m < n; ++m) tw[m] = make_double2((double)cosl(-2.0L * pi * m / n), (double)sinl(-2.0L * pi * m / n));
-    PCE_CUDA(c, cudaMalloc(&c->ztw, n * sizeof(double2)));
-    PCE_CUDA(c, cudaMemcpy(c->ztw, tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice));
+    std::vector<double2> tw;
+    stage_twiddles(n, tw);
+    PCE_CUDA(c, cudaMalloc(&c->ztw, tw.size() * sizeof(double2)));
+    PCE_CUDA(c, cudaMemcpy(c->ztw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice));
     // per-axis factors exp(-(1 - eta_d) k_d^2 / 4 xi^2) of eq. 26: [kx = 0..Nx/2 | ky = 0..Ny/2 | kz = 0..Nz/2]
     const int cnt[3] = {c->wk.Nxh, c->p.Ng[1] / 2 + 1, n / 2 + 1};
     std::vector<double> ze;
@@ -334,17 +215,6 @@ int zfft_scale(pce_ctx* c, const void* in, void* out, int deriv)
 {
     const double2* gin = static_cast<const double2*>(in);
     double2* gout = static_cast<double2*>(out);
-    static const bool pipe = [] { const char* e = getenv("PCE_ZFFT_PIPE"); return e && e[0] == '1'; }();
-    if (pipe && deriv < 0 && in == out && in == (const void*)c->gridk) {  // pipelined variant (persistent CTAs, cp.async double buffer): measured slower on B200 (fewer resident warps), kept for experiments
-        switch (c->p.Ng[2]) {
-            case 64: return launch_pipe<64>(c);
-            case 128: return launch_pipe<128>(c);
-            case 256: return launch_pipe<256>(c);
-            case 512: return launch_pipe<512>(c);
-            case 1024: return launch_pipe<1024>(c);
-            default: break;
-        }
-    }
     switch (c->p.Ng[2]) {
         case 16: return launch<16>(c, gin, gout, deriv);
         case 32: return launch<32>(c, gin, gout, deriv);
