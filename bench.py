@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-samples", type=int, nargs=2, default=None, help="two target counts for the oracle timing")
+    ap.add_argument("--bd", type=int, default=0, metavar="STEPS",
+                    help="also run STEPS Brownian-dynamics steps on the device (solve + forces + pce_bd_step; config 3: 100, dt = 1e-4 a^2)")
     return ap.parse_args()
 
 
@@ -312,6 +314,28 @@ def run_ours(args, rank, world, local_rank):
     flavours["m2_full_evaluation"] = {"ms": ms2, "per_s": 1e3 / ms2, "what": "psi and E at all N particles from all N charges"}
     flavours["per_step"] = {"m1": float(np.mean(iters)), "m2": 2.0}
 
+    # ---- optional: Brownian dynamics on the device: solve (cold / warm start) + forces + pce_bd_step per step
+    bd = None
+    if args.bd > 0 and w.N_ion > 0:
+        dt_bd = 1e-4 * w.a ** 2
+        bd = {"steps": args.bd, "dt": dt_bd, "what": "pce_solve + pce_forces + pce_bd_step per step, positions never leave the device"}
+        for mode in ("cold", "warm"):
+            ctx.set_positions(x, y, z)
+            qprev, its = None, []
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for s_ in range(args.bd):
+                qq, _, si = ctx.solve(Q, qi, w.E0, q0=qprev if mode == "warm" else None, allow_noconv=True)
+                oo = ctx.forces(qq, w.E0)
+                ctx.bd_step(oo["f"], dt_bd, 1.0, 1.0, seed=20240104 + args.config, step=s_)
+                qprev = qq
+                its.append(si["iters"])
+            b.record()
+            torch.cuda.synchronize()
+            bd[mode] = {"ms_per_step": a.elapsed_time(b) / args.bd, "cg_iters_mean": float(np.mean(its))}
+        ctx.set_positions(x, y, z)
+
     # ---- end to end through the host-buffer call (H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -367,13 +391,24 @@ def run_ours(args, rank, world, local_rank):
             d.update({"bound": "alu", "achieved": tf, "peak": dmma_tf, "unit": "TFLOP/s", "frac": tf / dmma_tf,
                       "hbm_achieved_gbs": gbs, "hbm_frac": gbs / hbm_peak, "algorithmic_fma": fma_per_launch})
         return d
+    # the (x, y) transforms (3-D transforms in mode 0) are cuFFT's unless the library runs its own passes (fftxy.cu)
+    fft_keys = ("fft_xy_forward(own)", "fft_xy_inverse(own)") if info["fft_mode"] == 2 else ("fft_d2z(cuFFT)", "ifft_z2d(cuFFT)")
+    fft_text = {0: "cuFFT 3-D D2Z/Z2D + separate scale pass",
+                1: "cuFFT 2-D D2Z/Z2D per mesh plane; the 'scale' pass is the fused z FFT + Green's function + inverse z FFT kernel",
+                2: "own (x, y) passes per mesh plane (fftxy.cu: one HBM trip per plane and direction); the 'scale' pass is the fused "
+                   "z FFT + Green's function + inverse z FFT kernel; no library call on the path"}[info["fft_mode"]]
+    # HBM ceiling of the bead-only matvec: the algorithmic bytes of all its passes at the measured copy rate
+    m1_bytes = (32 * w.N_bead + 8 * Ng3) + 2 * (8 * Ng3 + 16 * Nk) + 32 * Nk + (8 * Ng3 + 40 * w.N_bead) + 12 * info["nnz_near"] + 20 * w.N_bead
+    if "m1_bead_matvec" in flavours:
+        flavours["m1_bead_matvec"].update({"algorithmic_bytes": m1_bytes, "hbm_ceiling_per_s": hbm_peak * 1e9 / m1_bytes,
+                                           "frac_of_hbm_ceiling": flavours["m1_bead_matvec"]["per_s"] * m1_bytes / (hbm_peak * 1e9)})
     passes = {
         "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3, w.N_bead * P3),
         "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead, w.N_bead * P3),
         "real_bead_csr": rf(acc["bead_real"], nm1, 12 * info["nnz_near"] + 20 * w.N_bead),
         "scale": rf(acc["scale"], npairs, 32 * Nk),
-        "fft_d2z(cuFFT)": rf(acc["fft"], npairs, 8 * Ng3 + 16 * Nk),
-        "ifft_z2d(cuFFT)": rf(acc["ifft"], npairs, 8 * Ng3 + 16 * Nk),
+        fft_keys[0]: rf(acc["fft"], npairs, 8 * Ng3 + 16 * Nk),
+        fft_keys[1]: rf(acc["ifft"], npairs, 8 * Ng3 + 16 * Nk),
         "spread_full": rf(acc["spread"] - acc["bead_spread"], nfull, 32 * w.N + 8 * Ng3, w.N * P3),
         # per step: one potential-only gather at the beads (right-hand side) and one potential + field gather at all N
         "gather_full": rf(acc["gather"] - acc["bead_gather"], nfull, 8 * Ng3 + (40 * w.N_bead + 64 * w.N) / 2,
@@ -386,7 +421,7 @@ def run_ours(args, rank, world, local_rank):
     roof["peak_source"] = ("pce_measure_fp64_peaks (csrc/peaks.cu: fp64 mma.sync chains on this device, this run)" if roof["bound"] == "alu"
                            else peak_src)
     roof["traffic"] = None  # dram bytes per launch from the committed ncu --set full capture (config 5 only)
-    tpath = os.path.join(ROOT, "profiles", "r1f_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "r2_traffic.json")
     if args.config == 5 and os.path.exists(tpath):
         roof["traffic"] = json.load(open(tpath)).get(dom)
     line = {
@@ -395,8 +430,7 @@ def run_ours(args, rank, world, local_rank):
         "dtype": "f64", "data": "synthetic",
         "config": config_dict(w, args),
         "run_info": {"cells": info["ncell"], "nnz_near": info["nnz_near"],
-                     "fft": "cuFFT 2-D D2Z/Z2D per mesh plane; the 'scale' pass is the fused z FFT + Green's function + inverse z FFT kernel"
-                            if int(w.Ng[2]) in (16, 32, 64, 128, 256, 512, 1024) else "cuFFT 3-D D2Z/Z2D + separate scale pass"},
+                     "fft": fft_text},
         "counts": "value = (M1 bead-only solver matvecs + M2 full evaluations) / whole-step time; the flavours are split in 'flavours'",
         "flavours": flavours,
         "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
@@ -406,6 +440,8 @@ def run_ours(args, rank, world, local_rank):
         "roofline": roof, "roofline_passes": passes,
         "fp64_peaks_tflops": {"dfma": dfma_tf, "mma_f64": dmma_tf, "how": "pce_measure_fp64_peaks: register-resident chains, this device, this run"}, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
     }
+    if bd:
+        line["bd"] = bd
     if not args.no_cpu_baseline:
         import oracle as orc
         orc.build()

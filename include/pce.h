@@ -107,6 +107,7 @@ typedef struct {
     long long bytes_workspace;
     long long bytes_precond; /* fp32 storage of the block-Jacobi preconditioner (0: off) */
     int n_precond_blocks;    /* bodies that own a dense preconditioner block */
+    int fft_mode;            /* 0: cuFFT 3-D plans + scaling pass; 1: cuFFT 2-D per plane + fused z pass; 2: own (x, y) passes + fused z pass */
 } pce_info;
 
 /* Ewald parameters from a target tolerance (pure host arithmetic):

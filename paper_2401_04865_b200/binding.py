@@ -53,7 +53,7 @@ class PceTimings(C.Structure):
 class PceInfo(C.Structure):
     _fields_ = [("eta", C.c_double * 3), ("h", C.c_double * 3), ("ncell", C.c_int * 3), ("image_range", C.c_int * 3),
                 ("nnz_near", C.c_longlong), ("N", C.c_int), ("N_bead", C.c_int), ("N_body", C.c_int),
-                ("bytes_workspace", C.c_longlong), ("bytes_precond", C.c_longlong), ("n_precond_blocks", C.c_int)]
+                ("bytes_workspace", C.c_longlong), ("bytes_precond", C.c_longlong), ("n_precond_blocks", C.c_int), ("fft_mode", C.c_int)]
 
 
 class PceError(RuntimeError):
@@ -327,7 +327,7 @@ class Context:
         self._ck(self.lib.pce_get_info(self.h, C.byref(i)))
         return {"eta": list(i.eta), "h": list(i.h), "ncell": list(i.ncell), "image_range": list(i.image_range),
                 "nnz_near": i.nnz_near, "N": i.N, "N_bead": i.N_bead, "N_body": i.N_body, "bytes_workspace": i.bytes_workspace,
-                "bytes_precond": i.bytes_precond, "n_precond_blocks": i.n_precond_blocks}
+                "bytes_precond": i.bytes_precond, "n_precond_blocks": i.n_precond_blocks, "fft_mode": i.fft_mode}
 
     def launch_count(self):
         return int(self.lib.pce_launch_count(self.h))

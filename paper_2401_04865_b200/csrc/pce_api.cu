@@ -635,6 +635,7 @@ extern "C" int pce_get_info(const pce_ctx* c, pce_info* info)
     info->bytes_workspace = c->bytes;
     info->bytes_precond = c->pc_bytes;
     info->n_precond_blocks = c->pc_on ? c->pc_nblock : 0;
+    info->fft_mode = c->use_fftxy ? 2 : c->use_zfft ? 1 : 0;
     return PCE_OK;
 }
 
