@@ -156,19 +156,20 @@ __global__ void k_cell_scatter(int n, const int* __restrict__ cell_of, const int
     perm[cell_start[cidx] + slot] = i;
 }
 
-// one warp per cell: order the cell's entries by caller index (rank by counting)
-__global__ void k_cell_rank(int ncell, const int* __restrict__ cell_start, const int* __restrict__ perm_in, int* __restrict__ perm_out)
+// order every cell's entries by caller index (rank by counting): one thread per sorted slot, so that a crowded cell -- a
+// 2562-bead sphere inside a few cells -- is shared by as many threads as it has entries (one warp per cell took n_cell^2 / 32 steps)
+__global__ void __launch_bounds__(256)
+k_cell_rank(int n, const int* __restrict__ cell_of, const int* __restrict__ cell_start, const int* __restrict__ perm_in,
+            int* __restrict__ perm_out)
 {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (warp >= ncell) return;
-    const int b = cell_start[warp], e = cell_start[warp + 1];
-    for (int i = b + lane; i < e; i += 32) {
-        const int mine = perm_in[i];
-        int rank = 0;
-        for (int j = b; j < e; ++j) rank += (perm_in[j] < mine);
-        perm_out[b + rank] = mine;
-    }
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int mine = perm_in[s];
+    const int cidx = cell_of[mine];
+    const int b = cell_start[cidx], e = cell_start[cidx + 1];
+    int rank = 0;
+    for (int j = b; j < e; ++j) rank += (__ldg(perm_in + j) < mine);
+    perm_out[b + rank] = mine;
 }
 
 __global__ void k_iota(int n, int* p)
@@ -276,7 +277,7 @@ int bins_build(pce_ctx* c, Bins& b, const double* x, const double* y, const doub
         int rc = exclusive_scan(c, b.cell_start, b.ncell + 1);
         if (rc) return rc;
         k_cell_scatter<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.cell_of, b.cell_start, b.cell_fill, b.perm_tmp);
-        k_cell_rank<<<cdiv((long long)b.ncell * 32, 256), 256, 0, c->st>>>(b.ncell, b.cell_start, b.perm_tmp, b.perm);
+        k_cell_rank<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.cell_of, b.cell_start, b.perm_tmp, b.perm);
         c->launches += 2;
     }
     k_gather3<<<cdiv(n, 256), 256, 0, c->st>>>(n, b.perm, x, y, z, b.xs, b.ys, b.zs, b.inv);

@@ -121,11 +121,15 @@ __device__ __forceinline__ void pair_eval(const RealConst& k, const RealTable& T
 // times per stage instead of once per candidate.  Targets and sources may be different subsets with the same cell
 // geometry (targets = beads, sources = all, for the right-hand side of eq. 13).  A source at r = 0 -- the target
 // itself (the beta = alpha, n = 0 term) or a coincident particle (reading A9) -- contributes R(0) q (eq. 21) and no field.
-constexpr int RS_WARPS = 4;
+constexpr int RS_WARPS = 4;        // warps per CTA, a chunk per warp
+constexpr int RS_SPLIT_WARPS = 8;  // warps per CTA when the CTA shares one chunk (small systems)
 constexpr int RS_STAGE = 64;
 
-template <bool FIELD>
-__global__ void __launch_bounds__(RS_WARPS * 32)
+// SPLIT = 1: a warp per chunk.  SPLIT = WARPS (few chunks: small systems, where one warp walking ~1000 candidates per target is
+// the critical path of the whole launch): the CTA owns the chunk, warp w takes every WARPS-th source stage, the partial sums
+// are added in warp order (deterministic).
+template <bool FIELD, int WARPS, int SPLIT>
+__global__ void __launch_bounds__(WARPS * 32)
 k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_start, const int* __restrict__ t_chunk,
              const double* __restrict__ txs,
              const double* __restrict__ tys, const double* __restrict__ tzs, const int* __restrict__ s_start,
@@ -133,8 +137,8 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
              const double* __restrict__ sqs, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
              double* __restrict__ ez, int* __restrict__ work_ctr, int tab_in_smem)
 {
-    __shared__ double2 sh_xy[RS_WARPS][RS_STAGE];
-    __shared__ double2 sh_zq[RS_WARPS][RS_STAGE];
+    __shared__ double2 sh_xy[WARPS][RS_STAGE];
+    __shared__ double2 sh_zq[WARPS][RS_STAGE];
     extern __shared__ double sh_tab[];  // copy of the kernel table (potential rows, with FIELD also the field rows)
     if (tab_in_smem) {
         const int nt = (FIELD ? RT_STRIDE : RT_DEG + 1) * T.n_int;
@@ -145,13 +149,22 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double2* sxy = sh_xy[warp];
     double2* szq = sh_zq[warp];
+    __shared__ int sh_item;
+    __shared__ double sh_part[SPLIT > 1 ? WARPS : 1][4][32];
     const int ncell = g.nc[0] * g.nc[1] * g.nc[2];
     for (;;) {
         // work item: one chunk of up to 32 targets of ONE cell (cells.cu scans ceil(n_cell/32) into t_chunk): a crowded cell
         // is shared by many warps, a warp never straddles cells
         int item = 0;
-        if (lane == 0) item = atomicAdd(work_ctr, 1);
-        item = __shfl_sync(0xffffffffu, item, 0);
+        if (SPLIT > 1) {
+            __syncthreads();  // the previous item's partial sums are consumed
+            if (threadIdx.x == 0) sh_item = atomicAdd(work_ctr, 1);
+            __syncthreads();
+            item = sh_item;
+        } else {
+            if (lane == 0) item = atomicAdd(work_ctr, 1);
+            item = __shfl_sync(0xffffffffu, item, 0);
+        }
         if (item >= t_chunk[ncell]) return;
         int lo = 0, hi = ncell;  // largest cell with t_chunk[cell] <= item
         while (hi - lo > 1) {
@@ -163,6 +176,7 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
         const bool valid = i < t_start[cell + 1];
         const double xi = valid ? txs[i] : 1e150, yi = valid ? tys[i] : 1e150, zi = valid ? tzs[i] : 1e150;
         double a_psi = 0.0, a_x = 0.0, a_y = 0.0, a_z = 0.0;
+        int stage_id = 0;
         {
             const int cx = cell % g.nc[0], cy = (cell / g.nc[0]) % g.nc[1], cz = cell / (g.nc[0] * g.nc[1]);
             for (int oz = -g.range[2]; oz <= g.range[2]; ++oz) {
@@ -183,6 +197,7 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
                         const int scell = (nz * g.nc[1] + ny) * g.nc[0] + nx;
                         const int jb = s_start[scell], je = s_start[scell + 1];
                         for (int j0 = jb; j0 < je; j0 += RS_STAGE) {
+                            if (SPLIT > 1 && (stage_id++ % SPLIT) != warp) continue;
                             const int cnt = min(RS_STAGE, je - j0);
                             __syncwarp();
 #pragma unroll
@@ -224,6 +239,19 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
                 }
             }
         }
+        if (SPLIT > 1) {
+            sh_part[warp][0][lane] = a_psi;
+            if (FIELD) { sh_part[warp][1][lane] = a_x; sh_part[warp][2][lane] = a_y; sh_part[warp][3][lane] = a_z; }
+            __syncthreads();
+            if (warp != 0) continue;
+            a_psi = sh_part[0][0][lane];
+            if (FIELD) { a_x = sh_part[0][1][lane]; a_y = sh_part[0][2][lane]; a_z = sh_part[0][3][lane]; }
+#pragma unroll
+            for (int w = 1; w < SPLIT; ++w) {
+                a_psi += sh_part[w][0][lane];
+                if (FIELD) { a_x += sh_part[w][1][lane]; a_y += sh_part[w][2][lane]; a_z += sh_part[w][3][lane]; }
+            }
+        }
         if (valid) {
             psi[i] = a_psi * k.inv_eps;
             if (FIELD) { ex[i] = a_x * k.inv_eps; ey[i] = a_y * k.inv_eps; ez[i] = a_z * k.inv_eps; }
@@ -253,15 +281,20 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
     int blocks = c->num_sm * (per_sm < 1 ? 1 : per_sm > 8 ? 8 : per_sm);
     const int need = cdiv(cdiv(tb.n, 32) + tb.ncell, RS_WARPS);  // upper bound of the number of chunks
     if (blocks > need) blocks = need;
-    if (field) {
-        if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-        k_real_cells<true><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
-                                                                   sb.xs, sb.ys, sb.zs, sb.qs, psi_s, ex_s, ey_s, ez_s, c->work_ctr + 1, in_smem);
-    } else {
-        if (dyn > 40 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-        k_real_cells<false><<<blocks, RS_WARPS * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs, sb.cell_start,
-                                                                    sb.xs, sb.ys, sb.zs, sb.qs, psi_s, nullptr, nullptr, nullptr, c->work_ctr + 1, in_smem);
-    }
+    // few chunks (fewer than 4 per SM sub-partition): the CTA shares a chunk, one item per CTA
+    const int chunks_ub = cdiv(tb.n, 32) + tb.ncell;
+    const bool split = chunks_ub < c->num_sm * 16;
+    if (split) blocks = chunks_ub < c->num_sm * 4 ? chunks_ub : c->num_sm * 4;
+#define RS_LAUNCH(F, W, S)                                                                                                           \
+    do {                                                                                                                             \
+        if (dyn > 16 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<F, W, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn)); \
+        k_real_cells<F, W, S><<<blocks, W * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs,    \
+                                                              sb.cell_start, sb.xs, sb.ys, sb.zs, sb.qs, psi_s, F ? ex_s : nullptr,          \
+                                                              F ? ey_s : nullptr, F ? ez_s : nullptr, c->work_ctr + 1, in_smem);             \
+    } while (0)
+    if (field) { if (split) RS_LAUNCH(true, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH(true, RS_WARPS, 1); }
+    else { if (split) RS_LAUNCH(false, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH(false, RS_WARPS, 1); }
+#undef RS_LAUNCH
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
