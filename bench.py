@@ -447,7 +447,8 @@ def run_ours(args, rank, world, local_rank):
         orc.build()
         samples = tuple(args.cpu_samples) if args.cpu_samples else default_samples(w)
         t1, d1, _ = oracle_matvec_seconds(w, samples, "bead" if w.N_bead else "full")
-        line["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": d1,
+        line["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                                "sample": "direct-sum oracle (one M1 application: bead sources and targets, potential only), " + d1,
                                 "seconds_per_matvec": t1}
     print(json.dumps(line))
     if dist:

@@ -246,9 +246,10 @@ int pce_radial_profile(pce_ctx* ctx, int body, const double* q, double r_lo, int
 /* One whole pass of the hot path from HOST buffers (what bench.py's "e2e"
  * times): copy positions and charges to the device, rebuild cells, solve
  * eq. 13, evaluate forces, copy results back.  All pointers host; x,y,z [N];
- * outputs as in pce_solve / pce_forces (any output may be NULL). */
+ * outputs as in pce_solve / pce_forces (any output may be NULL).  warm_start != 0: the bead part of q (host, [N]) is
+ * read as the initial guess of the solve (e.g. the charges of the previous time step), as in pce_solve. */
 int pce_step_host(pce_ctx* ctx, const double* x, const double* y, const double* z,
-                  const double* Q_body, const double* q_ion, const double E0[3],
+                  const double* Q_body, const double* q_ion, const double E0[3], int warm_start,
                   double* q, double* Phi_body, double* fx, double* fy, double* fz,
                   double* F, double* T, double* S, double* U_tot, pce_solve_info* info);
 

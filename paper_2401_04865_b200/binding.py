@@ -88,7 +88,7 @@ def load():
     lib.pce_evaluate.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.pce_solve.argtypes = [vp, vp, vp, dp, C.c_int, vp, vp, C.POINTER(PceSolveInfo)]
     lib.pce_forces.argtypes = [vp, vp, dp] + [vp] * 9
-    lib.pce_step_host.argtypes = [vp, vp, vp, vp, vp, vp, dp] + [vp] * 9 + [C.POINTER(PceSolveInfo)]
+    lib.pce_step_host.argtypes = [vp, vp, vp, vp, vp, vp, dp, C.c_int] + [vp] * 9 + [C.POINTER(PceSolveInfo)]
     lib.pce_set_timing.argtypes = [vp, C.c_int]
     lib.pce_get_timings.argtypes = [vp, C.POINTER(PceTimings)]
     lib.pce_get_info.argtypes = [vp, C.POINTER(PceInfo)]
@@ -299,15 +299,15 @@ class Context:
         self._ck(self.lib.pce_radial_profile(self.h, int(body), _ptr(q), float(r_lo), int(n_bins), _ptr(counts), _ptr(g), _ptr(rho), _ptr(Qc)))
         return {"counts": counts.view(2, n_bins).T, "g": g.view(2, n_bins).T, "rho": rho, "Qcum": Qc}
 
-    def step_host(self, x, y, z, Q_body, q_ion, E0, out):
+    def step_host(self, x, y, z, Q_body, q_ion, E0, out, warm_start=False):
         """Host-buffer pass.  x,y,z,Q_body,q_ion: host numpy/pinned-torch f64; ``out``: dict of host arrays
-        (keys q, Phi, fx, fy, fz, F, T, S, U) written in place."""
+        (keys q, Phi, fx, fy, fz, F, T, S, U) written in place; warm_start: out["q"] holds the initial guess."""
         def hp(a):
             if a is None:
                 return None
             return C.c_void_p(a.data_ptr()) if hasattr(a, "data_ptr") else C.c_void_p(a.ctypes.data)
         info = PceSolveInfo()
-        rc = self._ck(self.lib.pce_step_host(self.h, hp(x), hp(y), hp(z), hp(Q_body), hp(q_ion), _d3(E0), hp(out.get("q")),
+        rc = self._ck(self.lib.pce_step_host(self.h, hp(x), hp(y), hp(z), hp(Q_body), hp(q_ion), _d3(E0), int(bool(warm_start)), hp(out.get("q")),
                                              hp(out.get("Phi")), hp(out.get("fx")), hp(out.get("fy")), hp(out.get("fz")),
                                              hp(out.get("F")), hp(out.get("T")), hp(out.get("S")), hp(out.get("U")),
                                              C.byref(info)), allow=(PCE_ENOCONV,))

@@ -558,12 +558,13 @@ extern "C" int pce_effective_permittivity(pce_ctx* c, double eps_eff[9], pce_sol
 
 // ---------------------------------------------------------------- host-buffer pass (bench "e2e")
 extern "C" int pce_step_host(pce_ctx* c, const double* x, const double* y, const double* z, const double* Q_body, const double* q_ion,
-                             const double E0[3], double* q, double* Phi_body, double* fx, double* fy, double* fz, double* F, double* T,
-                             double* S, double* U_tot, pce_solve_info* info)
+                             const double E0[3], int warm_start, double* q, double* Phi_body, double* fx, double* fy, double* fz, double* F,
+                             double* T, double* S, double* U_tot, pce_solve_info* info)
 {
     if (!c) return PCE_EINVAL;
     if (!c->have_system) { c->err = "pce_step_host before pce_set_system"; return PCE_ESTATE; }
     if (!x || !y || !z || !E0 || (c->Nbody > 0 && !Q_body) || (c->Nion > 0 && !q_ion)) { c->err = "NULL argument"; return PCE_EINVAL; }
+    if (warm_start && !q) { c->err = "pce_step_host: warm start needs q"; return PCE_EINVAL; }
     const size_t N = c->N, nb = c->Nbody, ni = c->Nion;
     const size_t need = 3 * N + nb + ni + N + nb + 3 * N + 9 * nb + 3 + 8;
     if (need > c->hs_dev_n) {
@@ -582,10 +583,11 @@ extern "C" int pce_step_host(pce_ctx* c, const double* x, const double* y, const
     PCE_CUDA(c, cudaMemcpyAsync(dz, z, N * 8, cudaMemcpyHostToDevice, c->st));
     if (nb) PCE_CUDA(c, cudaMemcpyAsync(dQ, Q_body, nb * 8, cudaMemcpyHostToDevice, c->st));
     if (ni) PCE_CUDA(c, cudaMemcpyAsync(dqi, q_ion, ni * 8, cudaMemcpyHostToDevice, c->st));
+    if (warm_start && c->Nbead) PCE_CUDA(c, cudaMemcpyAsync(dq, q, (size_t)c->Nbead * 8, cudaMemcpyHostToDevice, c->st));
     int rc = positions_impl(c, dx, dy, dz);
     int rc_solve = PCE_OK;
     if (!rc) {
-        rc_solve = solve_cg(c, dQ, dqi, E0, 0, dq, dPhi, info);
+        rc_solve = solve_cg(c, dQ, dqi, E0, warm_start ? 1 : 0, dq, dPhi, info);
         if (rc_solve != PCE_OK && rc_solve != PCE_ENOCONV) rc = rc_solve;
     }
     if (!rc) rc = forces_all(c, dq, E0, dfx, dfy, dfz, dF, dT, dS, nullptr, dU, nullptr);

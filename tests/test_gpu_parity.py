@@ -282,6 +282,9 @@ def test_step_host_matches_the_device_calls(pce):
         ref = out[key].cpu().numpy()
         assert np.abs(host[key].reshape(3, nb).T - ref).max() <= 1e-12 * max(np.abs(out["f"].cpu().numpy()).sum(0).max(), 1.0)
     assert host["U"][1] == pytest.approx(float(out["W"]), rel=1e-12)
+    # warm start from the converged charges (host["q"] is read as the initial guess): nothing left to iterate, same answer
+    sw = ctx.step_host(xs[0], xs[1], xs[2], np.ascontiguousarray(w.Q_body), np.ascontiguousarray(w.q_ion), w.E0, host, warm_start=True)
+    assert sw["converged"] and sw["iters"] <= 1 and rel(host["q"], q.cpu().numpy()) < 1e-11
     ctx.close()
 
 
