@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-samples", type=int, nargs=2, default=None, help="two target counts for the oracle timing")
+    ap.add_argument("--deterministic", action="store_true", help="PCE_FLAG_DETERMINISTIC: bit-reproducible gather (no fp64 atomics)")
     ap.add_argument("--bd", type=int, default=0, metavar="STEPS",
                     help="also run STEPS Brownian-dynamics steps on the device (solve + forces + pce_bd_step; config 3: 100, dt = 1e-4 a^2)")
     return ap.parse_args()
@@ -231,7 +232,7 @@ def run_ours(args, rank, world, local_rank):
     if dist:
         dist.barrier()
     w = make_workload(args.config, rank)
-    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver)
+    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, deterministic=args.deterministic)
     x, y, z, Q, qi = pce.upload(w)
     ctx.set_system(w.body_offset, x, y, z)
     info = ctx.info()
@@ -429,7 +430,7 @@ def run_ours(args, rank, world, local_rank):
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": config_dict(w, args),
-        "run_info": {"cells": info["ncell"], "nnz_near": info["nnz_near"],
+        "run_info": {"cells": info["ncell"], "nnz_near": info["nnz_near"], "deterministic_gather": bool(args.deterministic),
                      "fft": fft_text},
         "counts": "value = (M1 bead-only solver matvecs + M2 full evaluations) / whole-step time; the flavours are split in 'flavours'",
         "flavours": flavours,

@@ -62,6 +62,11 @@ typedef enum {
                                   transforms, wave-space momentum conserved to rounding) instead of the gradient of the gather
                                   window (default, one transform pair; reading A3). */
 
+#define PCE_FLAG_DETERMINISTIC 8 /* bit-reproducible results: the gather writes one partial per (brick, particle) pair and adds each
+                                  particle's partials in a fixed order instead of issuing fp64 atomics (the only run-to-run
+                                  variation of the library, at the 1e-16 level); costs memory (8 B per pair and quantity) and
+                                  ~15 % of the gather time.  Needs a mesh on the brick lattice (N_g % 8 == 0, N_g - P >= 8) */
+
 /* Parameters of the spectral Ewald sum and of the solver.
  * eta is NOT a free input: eta = h^2 xi^2 P / pi (eq. 31,
  * PAPER.md:250), per dimension for a rectangular box. */

@@ -336,12 +336,13 @@ class Context:
 PCE_FLAG_NO_PRECOND = 1
 PCE_FLAG_CUFFT_3D = 2
 PCE_FLAG_FIELD_IK = 4
+PCE_FLAG_DETERMINISTIC = 8
 
 
-def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None, precond=True, fused_z=True, field_ik=False) -> Context:
+def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None, precond=True, fused_z=True, field_ik=False, deterministic=False) -> Context:
     """Context with parameters suggested for a workloads.Workload."""
     p = suggest_params(workload.L, workload.Ng, workload.a, tol, P)
-    p.flags = (0 if precond else PCE_FLAG_NO_PRECOND) | (0 if fused_z else PCE_FLAG_CUFFT_3D) | (PCE_FLAG_FIELD_IK if field_ik else 0)
+    p.flags = (0 if precond else PCE_FLAG_NO_PRECOND) | (0 if fused_z else PCE_FLAG_CUFFT_3D) | (PCE_FLAG_FIELD_IK if field_ik else 0) | (PCE_FLAG_DETERMINISTIC if deterministic else 0)
     p.eps_f = workload.eps_f
     p.tol_solver = tol_solver
     p.max_iter = max_iter

@@ -98,7 +98,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     free_system(c);
     krylov_free(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape); cudaFree(c->xytw); cudaFree(c->xy_ctr);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape); cudaFree(c->xytw); cudaFree(c->xy_ctr); cudaFree(c->gather_part);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -186,6 +186,10 @@ static int create_impl(pce_ctx* c)
     int rcw = wave_bricks_init(c);
     if (rcw) return rcw;
     c->use_cols = wave_cols_supported(c);
+    if ((p.flags & PCE_FLAG_DETERMINISTIC) && !c->use_cols) {
+        c->err = "PCE_FLAG_DETERMINISTIC needs a mesh on the brick lattice (N_g % 8 == 0, N_g - P >= 8)";
+        return PCE_EINVAL;
+    }
     if (c->use_cols && (rcw = wave_cols_init(c))) return rcw;
     return realtab_upload(c);
 }

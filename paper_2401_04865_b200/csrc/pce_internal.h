@@ -62,6 +62,12 @@ struct Bins {
     int* col_arrive = nullptr;    // [ncell] arrival counters of split bricks
     double* qs_cols = nullptr;    // &hrec[0].q: charges are written into the records (stride 16 doubles)
     int col_chunk = 0, n_items = 0;
+    // deterministic gather (PCE_FLAG_DETERMINISTIC): pair numbering per brick, per-particle pair lists
+    int* pair_start = nullptr;    // [ncell + 1]
+    int* inv_ptr = nullptr;       // [n + 1]
+    int* inv_list = nullptr;      // [inv_cap] pair ids of each particle in a fixed order
+    int n_pairs = 0;
+    long long inv_cap = 0;
     long long col_ent_cap = 0, col_item_cap = 0, nkeys = 0;
 };
 
@@ -160,6 +166,8 @@ struct pce_ctx {
     bool use_cols = false;     // cached-list spread / gather (wave_cols.cu) instead of the per-call candidate walk
     int occ_cspread = 0, occ_cgather = 0, occ_cgather_f = 0;
     int* work_ctr = nullptr;
+    double* gather_part = nullptr;  // per-(brick, hit) partial sums of the deterministic gather
+    long long part_cap = 0;
 
     // per-call work vectors
     double *w_real = nullptr, *w_wave = nullptr;            // [N] sorted-order potentials

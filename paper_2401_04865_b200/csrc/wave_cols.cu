@@ -460,8 +460,11 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
               int n_items, const int* __restrict__ item_start, const HitRec* __restrict__ rec, const double4* __restrict__ u0g,
               const double* __restrict__ grid,
               double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey, double* __restrict__ ez,
-              int* __restrict__ work_ctr, const int* __restrict__ skip)
+              int* __restrict__ work_ctr, const int* __restrict__ skip, const int* __restrict__ pair_start, double* __restrict__ part,
+              long long part_stride)
 {
+    // pair_start != nullptr (PCE_FLAG_DETERMINISTIC): the contribution of hit h of brick b goes to part[pair_start[b] + h] (one
+    // plain store per pair and quantity) and k_gather_finish adds each particle's pairs in a fixed order; else one atomicAdd
     if (skip && *skip) return;
     if (items) n_items = item_start[g.nbx * g.nby * g.nbz];
     constexpr int STRIDE = FIELD ? STRIDE_FLD : STRIDE_PSI;
@@ -499,6 +502,7 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
             __syncwarp();
             batch_weights<FIELD, STRIDE, DW, 8>(wc, tab, it, s, nh, lane, false, u_cur);
             const int p_mine = p_cur;  // slot of hit hb + lane (output index)
+            const long long pair0 = pair_start ? (long long)pair_start[it.brick] + hb : 0;
             p_cur = p_next; u_cur = u_next;
             if (hb + 32 < it.h1) {
                 prefetch_records(s.rec, rec, p_next, lane);
@@ -543,7 +547,10 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                     double r = fma(wx2.y, u1, wx2.x * u0);
                     r += __shfl_xor_sync(0xffffffffu, r, 1);
                     r += __shfl_xor_sync(0xffffffffu, r, 2);
-                    if (live && t == 0) atomicAdd(&psi[po], r);
+                    if (live && t == 0) {
+                        if (pair_start) part[pair0 + hr] = r;
+                        else atomicAdd(&psi[po], r);
+                    }
                 } else {
                     const double b0 = live ? w[DW + BR + t] : 0.0, b1 = live ? w[DW + BR + t + 4] : 0.0;  // wy u_y
                     const double2 wxu2 = *reinterpret_cast<const double2*>(w + BR + 2 * t);               // wx u_x
@@ -585,16 +592,97 @@ k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
                     r0 += __shfl_xor_sync(0xffffffffu, r0, 2); r1 += __shfl_xor_sync(0xffffffffu, r1, 2);
                     r2 += __shfl_xor_sync(0xffffffffu, r2, 2); r3 += __shfl_xor_sync(0xffffffffu, r3, 2);
                     if (live) {  // E = -grad_a, dW/dx_a = +grad_fac u W; lane t issues quantity t
-                        if (t == 0) atomicAdd(&psi[po], r0);
-                        else if (t == 1) atomicAdd(&ex[po], -wc.grad_fac[0] * r1);
-                        else if (t == 2) atomicAdd(&ey[po], -wc.grad_fac[1] * r2);
-                        else atomicAdd(&ez[po], -wc.grad_fac[2] * r3);
+                        const double val = (t == 0) ? r0 : (t == 1) ? -wc.grad_fac[0] * r1 : (t == 2) ? -wc.grad_fac[1] * r2 : -wc.grad_fac[2] * r3;
+                        if (pair_start) part[(long long)t * part_stride + pair0 + hr] = val;
+                        else atomicAdd((t == 0) ? &psi[po] : (t == 1) ? &ex[po] : (t == 2) ? &ey[po] : &ez[po], val);
                     }
                 }
             }
             __syncwarp();
         }
     }
+}
+
+// ---------------------------------------------------------------- deterministic gather (PCE_FLAG_DETERMINISTIC)
+// pairs (brick, hit) are numbered pair_start[brick] + h; particle p meets the bricks (fx + i, fy + j, fz + k) of its support in a
+// fixed enumeration, so the slot of a pair in the particle's list follows from the brick coordinates alone: no atomics, no sort
+__global__ void __launch_bounds__(256)
+k_pair_count(int nbrick, ColGeom g, const int* __restrict__ key_start, int* __restrict__ pair_start)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b > nbrick) return;
+    int v = 0;
+    if (b < nbrick) {
+        int a0, n0, a1, n1;
+        brick_runs(g, key_start, b, a0, n0, a1, n1);
+        v = n0 + n1;
+    }
+    pair_start[b] = v;
+}
+
+__device__ __forceinline__ void brick_span(int s0, int P, int& f, int& cnt)
+{
+    f = s0 >> 3;  // floor for negatives too
+    cnt = ((s0 + P - 1) >> 3) - f + 1;
+}
+
+__global__ void __launch_bounds__(256)
+k_inv_count(int n, int P, const HitRec* __restrict__ rec, int* __restrict__ inv_ptr)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    int v = 0;
+    if (i < n) {
+        const int4 s0 = rec[i].s0;
+        int f, cx, cy, cz;
+        brick_span(s0.x, P, f, cx); brick_span(s0.y, P, f, cy); brick_span(s0.z, P, f, cz);
+        v = cx * cy * cz;
+    }
+    inv_ptr[i] = v;
+}
+
+// one warp per brick: pair (brick, h) -> slot in the list of its particle
+__global__ void __launch_bounds__(256)
+k_inv_fill(int nbrick, ColGeom g, const int* __restrict__ key_start, const int* __restrict__ ent, const HitRec* __restrict__ rec,
+           const int* __restrict__ pair_start, const int* __restrict__ inv_ptr, int* __restrict__ inv_list)
+{
+    const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (b >= nbrick) return;
+    int a0, n0, a1, n1;
+    brick_runs(g, key_start, b, a0, n0, a1, n1);
+    int t = b;
+    const int bx = t % g.nbx; t /= g.nbx;
+    const int by = t % g.nby, bz = t / g.nby;
+    const int base = pair_start[b];
+    for (int h = lane; h < n0 + n1; h += 32) {
+        const int p = ent[h < n0 ? a0 + h : a1 + (h - n0)];
+        const int4 s0 = rec[p].s0;
+        int fx, fy, fz, cx, cy, cz;
+        brick_span(s0.x, g.P, fx, cx); brick_span(s0.y, g.P, fy, cy); brick_span(s0.z, g.P, fz, cz);
+        int dx = (bx - fx) % g.nbx, dy = (by - fy) % g.nby, dz = (bz - fz) % g.nbz;
+        if (dx < 0) dx += g.nbx;
+        if (dy < 0) dy += g.nby;
+        if (dz < 0) dz += g.nbz;
+        inv_list[inv_ptr[p] + (dz * cy + dy) * cx + dx] = base + h;
+    }
+}
+
+// psi[p] = sum of the particle's pair contributions, in list order (fixed: bit-reproducible)
+__global__ void __launch_bounds__(256)
+k_gather_finish(int n, int nq, const int* __restrict__ inv_ptr, const int* __restrict__ inv_list, const double* __restrict__ part,
+                long long part_stride, double* __restrict__ o0, double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int b = inv_ptr[i], e = inv_ptr[i + 1];
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    for (int k = b; k < e; ++k) {
+        const long long g = inv_list[k];
+        a0 += __ldcg(part + g);
+        if (nq == 4) { a1 += __ldcg(part + part_stride + g); a2 += __ldcg(part + 2 * part_stride + g); a3 += __ldcg(part + 3 * part_stride + g); }
+    }
+    o0[i] = a0;
+    if (nq == 4) { o1[i] = a1; o2[i] = a2; o3[i] = a3; }
 }
 
 size_t smem_bytes(bool field)
@@ -659,6 +747,11 @@ int wave_cols_alloc(pce_ctx* c, Bins& b)
         PCE_CUDA(c, cudaMemsetAsync(b.col_arrive, 0, nbrick * sizeof(int), c->st));
         c->bytes += (long long)(b.col_item_cap * (8 + 4096) + nbrick * 4);
     }
+    if (c->p.flags & PCE_FLAG_DETERMINISTIC) {
+        PCE_CUDA(c, cudaMalloc(&b.pair_start, (nbrick + 1) * sizeof(int)));
+        PCE_CUDA(c, cudaMalloc(&b.inv_ptr, (n + 1) * sizeof(int)));
+        c->bytes += (long long)((nbrick + 1 + n + 1) * 4);
+    }
     b.nkeys = (long long)nkeys;
     b.qs_cols = reinterpret_cast<double*>(b.hrec) + 15;  // the charge sits in the last 8 bytes of every 128-byte record
     return PCE_OK;
@@ -668,6 +761,7 @@ void wave_cols_free(Bins& b)
 {
     cudaFree(b.hrec); cudaFree(b.wu0); cudaFree(b.col_cnt); cudaFree(b.col_start); cudaFree(b.col_ent); cudaFree(b.item_start);
     cudaFree(b.items); cudaFree(b.col_scratch); cudaFree(b.col_arrive);
+    cudaFree(b.pair_start); cudaFree(b.inv_ptr); cudaFree(b.inv_list);
 }
 
 // after bins_build: records and column lists of the binning's particles
@@ -697,6 +791,27 @@ int wave_cols_build(pce_ctx* c, Bins& b)
         k_item_fill<<<cdiv(b.ncell, 256), 256, 0, c->st>>>(b.ncell, b.item_start, b.items);
         c->launches++;
         b.n_items = (int)b.col_item_cap;  // upper bound (sizes the launch); the kernels read the count from item_start[ncell]
+    }
+    if (c->p.flags & PCE_FLAG_DETERMINISTIC) {  // pair numbering and the per-particle pair lists of the deterministic gather
+        k_pair_count<<<cdiv(b.ncell + 1, 256), 256, 0, c->st>>>(b.ncell, g, b.col_start, b.pair_start);
+        k_inv_count<<<cdiv(n + 1, 256), 256, 0, c->st>>>(n, g.P, b.hrec, b.inv_ptr);
+        c->launches += 2;
+        if ((rc = exclusive_scan(c, b.pair_start, b.ncell + 1))) return rc;
+        if ((rc = exclusive_scan(c, b.inv_ptr, n + 1))) return rc;
+        int totals[2] = {0, 0};
+        PCE_CUDA(c, cudaMemcpyAsync(&totals[0], b.pair_start + b.ncell, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+        PCE_CUDA(c, cudaMemcpyAsync(&totals[1], b.inv_ptr + n, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+        PCE_CUDA(c, cudaStreamSynchronize(c->st));
+        if (totals[0] != totals[1] || totals[0] < 0) { c->err = "deterministic gather: pair lists inconsistent (or more than 2^31 pairs)"; return PCE_EINVAL; }
+        b.n_pairs = totals[0];
+        if (b.n_pairs > b.inv_cap) {
+            cudaFree(b.inv_list);
+            b.inv_list = nullptr;
+            b.inv_cap = (long long)(b.n_pairs * 1.1) + 1024;
+            PCE_CUDA(c, cudaMalloc(&b.inv_list, (size_t)b.inv_cap * sizeof(int)));
+        }
+        k_inv_fill<<<cdiv((long long)b.ncell * 32, 256), 256, 0, c->st>>>(b.ncell, g, b.col_start, b.col_ent, b.hrec, b.pair_start, b.inv_ptr, b.inv_list);
+        c->launches++;
     }
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
@@ -729,21 +844,43 @@ int wave_gather_cols(pce_ctx* c, const Bins& b, bool field, double* psi_s, doubl
     if (b.n == 0) return PCE_OK;
     PassTimer t(c, PASS_GATHER);
     PCE_CUDA(c, cudaMemsetAsync(c->work_ctr, 0, sizeof(int), c->st));
-    PCE_CUDA(c, cudaMemsetAsync(psi_s, 0, (size_t)b.n * sizeof(double), c->st));
+    const bool det = (c->p.flags & PCE_FLAG_DETERMINISTIC) != 0;
+    const int nq = field ? 4 : 1;
+    const int* pair_start = nullptr;
+    if (det) {  // partial sums per (brick, hit) pair and quantity
+        const long long need = (long long)b.n_pairs * nq;
+        if (need > c->part_cap) {
+            cudaFree(c->gather_part);
+            c->gather_part = nullptr;
+            c->bytes -= c->part_cap * 8;
+            c->part_cap = need + need / 8 + 1024;
+            if (cudaMalloc(&c->gather_part, (size_t)c->part_cap * sizeof(double)) != cudaSuccess) { c->part_cap = 0; c->err = "out of device memory (gather partials)"; return PCE_ENOMEM; }
+            c->bytes += c->part_cap * 8;
+        }
+        pair_start = b.pair_start;
+    } else {
+        PCE_CUDA(c, cudaMemsetAsync(psi_s, 0, (size_t)b.n * sizeof(double), c->st));
+        if (field) {
+            PCE_CUDA(c, cudaMemsetAsync(ex_s, 0, (size_t)b.n * sizeof(double), c->st));
+            PCE_CUDA(c, cudaMemsetAsync(ey_s, 0, (size_t)b.n * sizeof(double), c->st));
+            PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
+        }
+    }
     const int2* items = b.col_chunk ? b.items : nullptr;
     if (field) {
-        PCE_CUDA(c, cudaMemsetAsync(ex_s, 0, (size_t)b.n * sizeof(double), c->st));
-        PCE_CUDA(c, cudaMemsetAsync(ey_s, 0, (size_t)b.n * sizeof(double), c->st));
-        PCE_CUDA(c, cudaMemsetAsync(ez_s, 0, (size_t)b.n * sizeof(double), c->st));
         k_gather_cols<true><<<grid_for(c, c->occ_cgather_f, b.n_items), CW * 32, smem_bytes(true), c->st>>>(
             c->wk, geom_of(c, b), b.col_start, b.col_ent, items, b.n_items, b.item_start, b.hrec, b.wu0, c->grid, psi_s, ex_s, ey_s, ez_s, c->work_ctr,
-            c->skip_flag);
+            c->skip_flag, pair_start, c->gather_part, (long long)b.n_pairs);
     } else {
         k_gather_cols<false><<<grid_for(c, c->occ_cgather, b.n_items), CW * 32, smem_bytes(false), c->st>>>(
             c->wk, geom_of(c, b), b.col_start, b.col_ent, items, b.n_items, b.item_start, b.hrec, b.wu0, c->grid, psi_s, nullptr, nullptr, nullptr, c->work_ctr,
-            c->skip_flag);
+            c->skip_flag, pair_start, c->gather_part, (long long)b.n_pairs);
     }
     c->launches++;
+    if (det) {
+        k_gather_finish<<<cdiv(b.n, 256), 256, 0, c->st>>>(b.n, nq, b.inv_ptr, b.inv_list, c->gather_part, (long long)b.n_pairs, psi_s, ex_s, ey_s, ez_s);
+        c->launches++;
+    }
     PCE_CUDA(c, cudaGetLastError());
     return PCE_OK;
 }

@@ -135,3 +135,37 @@ def test_set_centres_moves_the_reference_point_only():
     assert np.allclose(o1["S"].cpu().numpy(), S0 - d * w.Q_body[:, None], atol=1e-9 * np.abs(S0).max())
     assert np.allclose(o1["T"].cpu().numpy(), T0 - np.cross(d, F0), atol=1e-9 * max(np.abs(T0).max(), np.abs(F0).max()))
     ctx.close()
+
+
+def test_deterministic_flag_gives_bit_identical_results():
+    """PCE_FLAG_DETERMINISTIC (deterministic reductions): two evaluations and two solves of the same inputs
+    agree bit for bit, and with the oracle / the default (atomic) gather to the usual bars."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.config2(d=2.3)
+    rng = np.random.default_rng(8)
+    qv = torch.from_numpy(rng.normal(size=w.N)).cuda()
+    outs = []
+    for det in (True, True, False):
+        ctx = pce.context_for(w, deterministic=det)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        ev = [t.clone() for t in ctx.evaluate(qv)]
+        mv = ctx.matvec(qv[:w.N_bead].contiguous()).clone()
+        q, Phi, info = ctx.solve(Q, qi, w.E0)
+        f = ctx.forces(q, w.E0)
+        outs.append((ev, mv, q.clone(), f["f"].clone(), f["T"].clone()))
+        ctx.close()
+    a, b, c = outs
+    for u, v in zip(a[0] + [a[1], a[2], a[3], a[4]], b[0] + [b[1], b[2], b[3], b[4]]):
+        assert torch.equal(u, v)                                   # bit for bit
+    for u, v in zip(a[0] + [a[1], a[2]], c[0] + [c[1], c[2]]):
+        assert rel(u.cpu().numpy(), v.cpu().numpy()) < 1e-12       # the atomic gather differs by rounding only
+    psi_o, E_o = orc.ewald_eval(w.x, qv.cpu().numpy(), w.L, w.a)
+    assert rel(a[0][0].cpu().numpy(), psi_o) < 1e-9
+    assert rel(torch.stack(a[0][1:], dim=1).cpu().numpy(), E_o) < 1e-9
+    # a mesh off the brick lattice cannot honour the flag: refused at create
+    w2 = wl.tiny_random(seed=3, n_body=1, n_ion=10, L=6.0, Ng=36)
+    with pytest.raises(pce.PceError):
+        pce.context_for(w2, deterministic=True)
