@@ -110,7 +110,7 @@ typedef struct {
     long long nnz_near;     /* entries of the cached bead-bead near field */
     int    N, N_bead, N_body;
     long long bytes_workspace;
-    long long bytes_precond; /* fp32 storage of the block-Jacobi preconditioner (0: off) */
+    long long bytes_precond; /* storage of the block-Jacobi preconditioner (bf16 for many large bodies, else fp32; 0: off) */
     int n_precond_blocks;    /* bodies that own a dense preconditioner block */
     int fft_mode;            /* 0: cuFFT 3-D plans + scaling pass; 1: cuFFT 2-D per plane + fused z pass; 2: own (x, y) passes + fused z pass */
 } pce_info;

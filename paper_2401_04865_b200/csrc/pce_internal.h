@@ -189,7 +189,8 @@ struct pce_ctx {
     const int* skip_flag = nullptr;     // when set, the operator kernels return at once if *skip_flag != 0 (solver converged)
     // block-Jacobi preconditioner (precond.cu)
     bool pc_on = false;
-    float* pc_B = nullptr;            // per-body n_i x n_i fp32 blocks
+    void* pc_B = nullptr;             // per-body n_i x n_i blocks in bf16 or fp32, rows padded to 8 entries
+    bool pc_bf16 = false;
     void* pc_rows = nullptr;          // CTA -> (body, first row) map of the apply kernel
     unsigned char* pc_has = nullptr;  // [Nbody] 1 if the body has a dense block
     int pc_nrows_cta = 0, pc_max_n = 0, pc_nblock = 0;

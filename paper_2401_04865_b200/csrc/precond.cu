@@ -9,9 +9,11 @@
 //   B_i = A^-1 - u u^T / (1^T u),  u = A^-1 1
 // is the inverse of A on the zero-net-charge subspace of the body (the constraint sum_j q_ij = Q_i of eq. 11),
 // symmetric positive semi-definite with null vector 1.  The Krylov driver applies z = P B r (P = remove the
-// per-body mean) as one dense matrix-vector product per body.  B is stored in fp32 (it only steers the
-// search directions; every quantity that enters the result -- residual, step lengths, charges -- stays fp64),
-// which halves the HBM bytes of the apply: sum_i 4 n_i^2 bytes per iteration (2 GB at 500 x 1000 beads).
+// per-body mean) as one dense matrix-vector product per body.  B is stored in bf16 for large systems (it only steers the
+// search directions; every quantity that enters the result -- residual, step lengths, charges -- stays fp64;
+// measured: 30 iterations at config 5 with fp32, with 11 and with 8 mantissa bits alike), which quarters the HBM
+// bytes of the apply: sum_i 2 n_i^2 bytes per iteration (1 GB at 500 x 1000 beads).  Rows are padded to a multiple
+// of 8 entries (16-byte loads), rounding is to nearest even and symmetric (B_jk and B_kj round alike).
 //
 // Inversion: in-place block Gauss-Jordan without pivoting (every pivot block is a Schur complement of an SPD
 // matrix), 32 pivots per step.  Per step a panel kernel (reads A only; writes D^-1, the row panel D^-1 A_K:,
@@ -19,17 +21,20 @@
 // writer of A) run over all bodies of a chunk at once.
 #include "pce_internal.h"
 
+#include <cstdlib>
+
 constexpr int GJB = 32;            // pivots per block step
+__host__ __device__ constexpr int pc_ld(int n) { return (n + 7) & ~7; }  // row stride of the stored block (16-byte loads)
 constexpr int PC_MAX_BODY = 4096;  // larger bodies are left unpreconditioned (scaled identity)
 constexpr long long PC_CHUNK_ELEMS = 1ll << 28;  // fp64 work matrix per chunk of bodies: 2 GB
-constexpr long long PC_MAX_ELEMS = 3ll << 30;    // total fp32 storage cap: 12 GB
+constexpr long long PC_MAX_ELEMS = 3ll << 30;    // total bf16 storage cap: 6 GB
 
 struct PcBody {          // one preconditioned body inside the current chunk
     int j0, n;           // first bead, bead count
     int body, pad;       // body index
     long long woff;      // offset of its n x n fp64 work matrix
     long long poff;      // offset of its panels (3 x n x GJB + GJB x GJB doubles)
-    long long boff;      // offset of its fp32 matrix in pc_B
+    long long boff;      // offset (entries) of its matrix (row stride pc_ld(n)) in pc_B
 };
 
 // ---------------------------------------------------------------- A_jk = M_free(|r_j - r_k|), eq. 10
@@ -211,9 +216,10 @@ k_pc_usum(const PcBody* __restrict__ bodies, const double* __restrict__ u, doubl
 }
 
 // B_ij = (Ainv_ij + Ainv_ji)/2 - u_i u_j / s   -> fp32 (32x32 tiles, transposed read through shared memory)
+template <bool BF16>
 __global__ void __launch_bounds__(256)
 k_pc_final(const PcBody* __restrict__ bodies, const double* __restrict__ work, const double* __restrict__ u,
-           const double* __restrict__ usum, float* __restrict__ Bout)
+           const double* __restrict__ usum, void* __restrict__ Bout)
 {
     __shared__ double tT[32][33];
     const PcBody B = bodies[blockIdx.z];
@@ -229,7 +235,13 @@ k_pc_final(const PcBody* __restrict__ bodies, const double* __restrict__ work, c
         const int i = i0 + r, j = j0 + tx;
         if (i < n && j < n) {
             const double v = 0.5 * (A[(long long)i * n + j] + tT[tx][r]) - u[B.j0 + i] * u[B.j0 + j] * inv_s;
-            Bout[B.boff + (long long)i * n + j] = (float)v;
+            const long long o = B.boff + (long long)i * pc_ld(n) + j;
+            if (BF16) {
+                const unsigned u32 = __float_as_uint((float)v);
+                static_cast<unsigned short*>(Bout)[o] = (unsigned short)((u32 + 0x7fffu + ((u32 >> 16) & 1u)) >> 16);  // nearest even
+            } else {
+                static_cast<float*>(Bout)[o] = (float)v;
+            }
         }
     }
 }
@@ -239,44 +251,54 @@ struct PcRows { int j0, n, row0; int pad; long long boff; };  // CTA -> body, fi
 
 constexpr int PC_ROWS = 32;  // rows per CTA (4 per warp)
 
+__device__ __forceinline__ double bf16_lo(unsigned w) { return (double)__uint_as_float(w << 16); }
+__device__ __forceinline__ double bf16_hi(unsigned w) { return (double)__uint_as_float(w & 0xffff0000u); }
+
+template <bool BF16>
 __global__ void __launch_bounds__(256)
-k_pc_apply(const PcRows* __restrict__ rows, const float* __restrict__ Bm, const double* __restrict__ r, double* __restrict__ z,
+k_pc_apply(const PcRows* __restrict__ rows, const void* __restrict__ Bv, const double* __restrict__ r, double* __restrict__ z,
            const int* __restrict__ skip)
 {
     if (skip && *skip) return;  // solver already converged (krylov.cu)
-    extern __shared__ double sr[];  // the body's residual
+    extern __shared__ double sr[];  // the body's residual, zero-padded to the row stride
     const PcRows R = rows[blockIdx.x];
-    for (int j = threadIdx.x; j < R.n; j += 256) sr[j] = r[R.j0 + j];
+    const int ld = pc_ld(R.n);
+    for (int j = threadIdx.x; j < ld; j += 256) sr[j] = (j < R.n) ? r[R.j0 + j] : 0.0;
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool vec = (R.n % 4 == 0);
     // the warp's 4 rows are swept together: one read of the residual from shared memory serves 4 rows, and 4 independent
-    // 16-byte loads are in flight per lane
+    // 16-byte loads (8 entries each) are in flight per lane
     constexpr int NR = PC_ROWS / 8;
-    const float* Br[NR];
+    constexpr int ES = BF16 ? 2 : 4;   // bytes per stored entry
+    const unsigned char* Br[NR];
     bool live[NR];
     double acc[NR];
 #pragma unroll
     for (int k = 0; k < NR; ++k) {
         const int row = R.row0 + warp + 8 * k;
         live[k] = row < R.n;
-        Br[k] = Bm + R.boff + (long long)(live[k] ? row : 0) * R.n;
+        Br[k] = static_cast<const unsigned char*>(Bv) + (R.boff + (long long)(live[k] ? row : 0) * ld) * ES;
         acc[k] = 0.0;
     }
-    if (vec) {
-        for (int j = 4 * lane; j < R.n; j += 128) {
-            const double2 r01 = *reinterpret_cast<const double2*>(sr + j), r23 = *reinterpret_cast<const double2*>(sr + j + 2);
+    for (int j = 8 * lane; j < ld; j += 256) {
+        const double2 r01 = *reinterpret_cast<const double2*>(sr + j), r23 = *reinterpret_cast<const double2*>(sr + j + 2);
+        const double2 r45 = *reinterpret_cast<const double2*>(sr + j + 4), r67 = *reinterpret_cast<const double2*>(sr + j + 6);
 #pragma unroll
-            for (int k = 0; k < NR; ++k) {
-                const float4 b = *reinterpret_cast<const float4*>(Br[k] + j);
-                acc[k] = fma((double)b.x, r01.x, fma((double)b.y, r01.y, fma((double)b.z, r23.x, fma((double)b.w, r23.y, acc[k]))));
+        for (int k = 0; k < NR; ++k) {
+            double a = acc[k];
+            if (!BF16) {
+                const float4 b0 = __ldg(reinterpret_cast<const float4*>(Br[k] + (size_t)j * 4)), b1 = __ldg(reinterpret_cast<const float4*>(Br[k] + (size_t)j * 4 + 16));
+                a = fma((double)b0.x, r01.x, a); a = fma((double)b0.y, r01.y, a); a = fma((double)b0.z, r23.x, a); a = fma((double)b0.w, r23.y, a);
+                a = fma((double)b1.x, r45.x, a); a = fma((double)b1.y, r45.y, a); a = fma((double)b1.z, r67.x, a); a = fma((double)b1.w, r67.y, a);
+                acc[k] = a;
+                continue;
             }
-        }
-    } else {
-        for (int j = lane; j < R.n; j += 32) {
-            const double rj = sr[j];
-#pragma unroll
-            for (int k = 0; k < NR; ++k) acc[k] = fma((double)Br[k][j], rj, acc[k]);
+            const uint4 b = __ldg(reinterpret_cast<const uint4*>(Br[k] + (size_t)j * 2));
+            a = fma(bf16_lo(b.x), r01.x, a); a = fma(bf16_hi(b.x), r01.y, a);
+            a = fma(bf16_lo(b.y), r23.x, a); a = fma(bf16_hi(b.y), r23.y, a);
+            a = fma(bf16_lo(b.z), r45.x, a); a = fma(bf16_hi(b.z), r45.y, a);
+            a = fma(bf16_lo(b.w), r67.x, a); a = fma(bf16_hi(b.w), r67.y, a);
+            acc[k] = a;
         }
     }
 #pragma unroll
@@ -322,18 +344,23 @@ int precond_setup(pce_ctx* c)
         if (n < 2 || n > PC_MAX_BODY || total + (long long)n * n > PC_MAX_ELEMS) continue;
         PcBody B;
         B.j0 = off[b]; B.n = n; B.body = b; B.pad = 0; B.woff = 0; B.poff = 0; B.boff = total;
-        total += (long long)n * n;
-        total = (total + 3) & ~3ll;  // 16-byte aligned rows for float4 loads when n % 4 == 0
+        total += (long long)n * pc_ld(n);  // rows padded to 8 entries: 16-byte aligned for the uint4 loads
         all.push_back(B);
         has[b] = 1;
         if (n > max_n) max_n = n;
     }
     if (all.empty()) return PCE_OK;
-    if (cudaMalloc(&c->pc_B, (size_t)total * sizeof(float)) != cudaSuccess) {
+    // storage precision: bf16 where the apply is a real share of the iteration (many bodies, > 128 MB in fp32: the iteration
+    // count is set by the coupling between bodies, 30 at config 5 either way), fp32 for few or small bodies, whose blocks are
+    // nearly exact inverses of the whole operator (config 3: 3 iterations with fp32, 6 with bf16)
+    c->pc_bf16 = (int)all.size() >= 16 && total * 4 > (128ll << 20);
+    const size_t esize = c->pc_bf16 ? sizeof(unsigned short) : sizeof(float);
+    if (cudaMalloc(&c->pc_B, (size_t)total * esize) != cudaSuccess) {
         cudaGetLastError();
         c->pc_B = nullptr;
         return PCE_OK;  // no room for the preconditioner: plain CG (the result does not depend on it)
     }
+    PCE_CUDA(c, cudaMemsetAsync(c->pc_B, 0, (size_t)total * esize, c->st));  // the row padding must read as 0
     PCE_CUDA(c, cudaMalloc(&c->pc_has, (size_t)nb));
     PCE_CUDA(c, cudaMemcpyAsync(c->pc_has, has.data(), (size_t)nb, cudaMemcpyHostToDevice, c->st));
     // CTA -> (body, first row) map of the apply kernel
@@ -346,10 +373,13 @@ int precond_setup(pce_ctx* c)
     c->pc_nrows_cta = (int)rows.size();
     c->pc_max_n = max_n;
     c->pc_nblock = (int)all.size();
-    c->pc_bytes = total * (long long)sizeof(float);
+    c->pc_bytes = total * (long long)esize;
     c->bytes += c->pc_bytes;
-    if ((size_t)max_n * sizeof(double) > 48 * 1024)
-        PCE_CUDA(c, cudaFuncSetAttribute(k_pc_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(max_n * sizeof(double))));
+    if ((size_t)pc_ld(max_n) * sizeof(double) > 48 * 1024)
+    {
+        PCE_CUDA(c, cudaFuncSetAttribute(k_pc_apply<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(pc_ld(max_n) * sizeof(double))));
+        PCE_CUDA(c, cudaFuncSetAttribute(k_pc_apply<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(pc_ld(max_n) * sizeof(double))));
+    }
 
     // chunks of bodies whose fp64 work matrices fit PC_CHUNK_ELEMS
     double *work = nullptr, *panels = nullptr, *u = nullptr, *usum = nullptr;
@@ -398,7 +428,8 @@ int precond_setup(pce_ctx* c)
             }
             k_pc_rowsum<<<dim3(cdiv(nmax, 8), nbz), 256, 0, c->st>>>(bp, work, u);
             k_pc_usum<<<nbz, 256, 0, c->st>>>(bp, u, usum + b0, c->pc_invs);
-            k_pc_final<<<dim3(cdiv(nmax, 32), cdiv(nmax, 32), nbz), 256, 0, c->st>>>(bp, work, u, usum + b0, c->pc_B);
+            if (c->pc_bf16) k_pc_final<true><<<dim3(cdiv(nmax, 32), cdiv(nmax, 32), nbz), 256, 0, c->st>>>(bp, work, u, usum + b0, c->pc_B);
+            else k_pc_final<false><<<dim3(cdiv(nmax, 32), cdiv(nmax, 32), nbz), 256, 0, c->st>>>(bp, work, u, usum + b0, c->pc_B);
             c->launches += 3;
         }
         if (cudaStreamSynchronize(c->st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = PCE_ECUDA; c->err = "preconditioner set-up kernels failed"; }
@@ -418,7 +449,10 @@ int precond_setup(pce_ctx* c)
 int precond_apply(pce_ctx* c, const double* r, double* z)
 {
     if (!c->pc_on) return PCE_OK;
-    k_pc_apply<<<c->pc_nrows_cta, 256, (size_t)c->pc_max_n * sizeof(double), c->st>>>((const PcRows*)c->pc_rows, c->pc_B, r, z, c->skip_flag);
+    if (c->pc_bf16)
+        k_pc_apply<true><<<c->pc_nrows_cta, 256, (size_t)pc_ld(c->pc_max_n) * sizeof(double), c->st>>>((const PcRows*)c->pc_rows, c->pc_B, r, z, c->skip_flag);
+    else
+        k_pc_apply<false><<<c->pc_nrows_cta, 256, (size_t)pc_ld(c->pc_max_n) * sizeof(double), c->st>>>((const PcRows*)c->pc_rows, c->pc_B, r, z, c->skip_flag);
     c->launches++;
     if (c->pc_nblock < c->Nbody) {
         k_pc_identity<<<cdiv(c->Nbead, 256), 256, 0, c->st>>>(c->Nbead, c->pc_has, c->body_of, 4.0 * PCE_PI * c->p.eps_f * c->p.a, r, z, c->skip_flag);

@@ -95,10 +95,13 @@ __device__ __forceinline__ void for_neighbors(const CellGeom& g, const int* __re
 }
 
 // R(r) and g = -R'(r)/r (times eps_f) at s = r^2 > 0: table of realtab.h + closed-form Heaviside term; exact below s_lo
-__device__ __forceinline__ void pair_eval(const RealConst& k, const RealTable& T, double s, bool field, double& R, double& g)
+template <int NS = 0>
+__device__ __forceinline__ void pair_eval(const RealConst& k, const RealTable& T, double s, bool field, double& R, double& g,
+                                          const double* sh = nullptr)
 {
     if (s >= T.s_lo) {
-        rt_eval(T, s, field, R, g);
+        if (NS > 0) rt_eval_sh<NS>(sh, T.key_lo, s, field, R, g);
+        else rt_eval(T, s, field, R, g);
         if (s < k.two_a * k.two_a) {  // overlapping shells: Heaviside term of eq. 20 (reading G3)
             const double ir = rsqrt(s), r = s * ir, m = r - k.two_a;
             R -= m * m * k.t_lin * ir;                                      // t_lin = 1/(16 pi a^2)
@@ -128,23 +131,23 @@ constexpr int RS_STAGE = 64;
 // SPLIT = 1: a warp per chunk.  SPLIT = WARPS (few chunks: small systems, where one warp walking ~1000 candidates per target is
 // the critical path of the whole launch): the CTA owns the chunk, warp w takes every WARPS-th source stage, the partial sums
 // are added in warp order (deterministic).
-template <bool FIELD, int WARPS, int SPLIT>
+// NS > 0: the table sits in shared memory with the compile-time row stride NS (realtab.h); NS = 0: global memory, generic loads.
+template <bool FIELD, int WARPS, int SPLIT, int NS>
 __global__ void __launch_bounds__(WARPS * 32)
 k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_start, const int* __restrict__ t_chunk,
              const double* __restrict__ txs,
              const double* __restrict__ tys, const double* __restrict__ tzs, const int* __restrict__ s_start,
              const double* __restrict__ sxs, const double* __restrict__ sys, const double* __restrict__ szs,
              const double* __restrict__ sqs, double* __restrict__ psi, double* __restrict__ ex, double* __restrict__ ey,
-             double* __restrict__ ez, int* __restrict__ work_ctr, int tab_in_smem)
+             double* __restrict__ ez, int* __restrict__ work_ctr)
 {
     __shared__ double2 sh_xy[WARPS][RS_STAGE];
     __shared__ double2 sh_zq[WARPS][RS_STAGE];
-    extern __shared__ double sh_tab[];  // copy of the kernel table (potential rows, with FIELD also the field rows)
-    if (tab_in_smem) {
-        const int nt = (FIELD ? RT_STRIDE : RT_DEG + 1) * T.n_int;
-        for (int e = threadIdx.x; e < nt; e += blockDim.x) sh_tab[e] = T.tab[e];
+    extern __shared__ double sh_tab[];  // copy of the kernel table (potential rows, with FIELD also the field rows), row stride NS
+    if (NS > 0) {
+        constexpr int rows = FIELD ? RT_STRIDE : RT_DEG + 1;
+        for (int e = threadIdx.x; e < rows * T.n_int; e += blockDim.x) sh_tab[(e / T.n_int) * NS + e % T.n_int] = T.tab[e];
         __syncthreads();
-        T.tab = sh_tab;
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double2* sxy = sh_xy[warp];
@@ -227,7 +230,7 @@ k_real_cells(CellGeom g, RealConst k, RealTable T, const int* __restrict__ t_sta
                                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                                 if (r2 == 0.0) { a_psi = fma(k.R0, pzq.y, a_psi); continue; }  // eq. 21
                                 double R, gk = 0.0;
-                                pair_eval(k, T, r2, FIELD, R, gk);
+                                pair_eval<NS>(k, T, r2, FIELD, R, gk, sh_tab);
                                 a_psi = fma(R, pzq.y, a_psi);
                                 if (FIELD) {
                                     const double f = gk * pzq.y;
@@ -274,10 +277,10 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
         return PCE_OK;
     }
     PCE_CUDA(c, cudaMemsetAsync(c->work_ctr + 1, 0, sizeof(int), c->st));
-    const size_t tab_bytes = (size_t)(field ? RT_STRIDE : RT_DEG + 1) * c->rt.n_int * sizeof(double);
-    const int in_smem = tab_bytes <= 96 * 1024 ? 1 : 0;  // else the table is read from global memory (L1/L2)
-    const size_t dyn = in_smem ? tab_bytes : 0;
-    const int per_sm = in_smem ? (int)((200 * 1024) / (dyn + 8192 + 1024)) : 8;
+    // the table goes to shared memory with a compile-time row stride (192 or 320 intervals); larger tables stay in global memory
+    const int ns = c->rt.n_int <= 192 ? 192 : c->rt.n_int <= 320 ? 320 : 0;
+    const size_t dyn = (size_t)(field ? RT_STRIDE : RT_DEG + 1) * ns * sizeof(double);
+    const int per_sm = ns ? (int)((200 * 1024) / (dyn + 8192 + 1024)) : 8;
     int blocks = c->num_sm * (per_sm < 1 ? 1 : per_sm > 8 ? 8 : per_sm);
     const int need = cdiv(cdiv(tb.n, 32) + tb.ncell, RS_WARPS);  // upper bound of the number of chunks
     if (blocks > need) blocks = need;
@@ -285,15 +288,22 @@ int real_direct(pce_ctx* c, const Bins& tb, const Bins& sb, bool field, double* 
     const int chunks_ub = cdiv(tb.n, 32) + tb.ncell;
     const bool split = chunks_ub < c->num_sm * 16;
     if (split) blocks = chunks_ub < c->num_sm * 4 ? chunks_ub : c->num_sm * 4;
-#define RS_LAUNCH(F, W, S)                                                                                                           \
+#define RS_LAUNCH(F, W, S, NS)                                                                                                       \
     do {                                                                                                                             \
-        if (dyn > 16 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<F, W, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn)); \
-        k_real_cells<F, W, S><<<blocks, W * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs,    \
-                                                              sb.cell_start, sb.xs, sb.ys, sb.zs, sb.qs, psi_s, F ? ex_s : nullptr,          \
-                                                              F ? ey_s : nullptr, F ? ez_s : nullptr, c->work_ctr + 1, in_smem);             \
+        if (dyn > 16 * 1024) PCE_CUDA(c, cudaFuncSetAttribute(k_real_cells<F, W, S, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn)); \
+        k_real_cells<F, W, S, NS><<<blocks, W * 32, dyn, c->st>>>(geom_of(tb), c->rk, c->rt, tb.cell_start, tb.chunk_start, tb.xs, tb.ys, tb.zs, \
+                                                                  sb.cell_start, sb.xs, sb.ys, sb.zs, sb.qs, psi_s, F ? ex_s : nullptr,      \
+                                                                  F ? ey_s : nullptr, F ? ez_s : nullptr, c->work_ctr + 1);                  \
     } while (0)
-    if (field) { if (split) RS_LAUNCH(true, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH(true, RS_WARPS, 1); }
-    else { if (split) RS_LAUNCH(false, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH(false, RS_WARPS, 1); }
+#define RS_LAUNCH_NS(F, W, S)                                                  \
+    do {                                                                       \
+        if (ns == 192) RS_LAUNCH(F, W, S, 192);                                \
+        else if (ns == 320) RS_LAUNCH(F, W, S, 320);                           \
+        else RS_LAUNCH(F, W, S, 0);                                            \
+    } while (0)
+    if (field) { if (split) RS_LAUNCH_NS(true, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH_NS(true, RS_WARPS, 1); }
+    else { if (split) RS_LAUNCH_NS(false, RS_SPLIT_WARPS, RS_SPLIT_WARPS); else RS_LAUNCH_NS(false, RS_WARPS, 1); }
+#undef RS_LAUNCH_NS
 #undef RS_LAUNCH
     c->launches++;
     PCE_CUDA(c, cudaGetLastError());

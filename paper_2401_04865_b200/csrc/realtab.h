@@ -71,3 +71,30 @@ RT_HD void rt_eval(const RealTable& T, double s, bool field, double& N, double& 
         g = (p67 * t2 + p45) * t4 + (p23 * t2 + p01);
     }
 }
+
+#ifdef __CUDACC__
+// The same from a shared-memory copy laid out with a COMPILE-TIME row stride NS (>= n_int): every coefficient sits at a fixed
+// offset from the interval's first word, so the 8 (16 with the field) loads are LDS with immediate offsets -- through the
+// generic pointer and the run-time stride of rt_eval each load cost two 64-bit adds and a generic LD (38 % of the instructions
+// of the direct pass, ncu).
+template <int NS>
+__device__ __forceinline__ void rt_eval_sh(const double* sh, int key_lo, double s, bool field, double& N, double& g)
+{
+    const int hi = __double2hiint(s);
+    const int key = hi >> (20 - RT_BITS);
+    const double s0 = __hiloint2double(key << (20 - RT_BITS), 0);
+    const double two_inv_w = __hiloint2double((2047 + RT_BITS - (key >> RT_BITS)) << 20, 0);
+    const double t = (s - s0) * two_inv_w - 1.0;
+    const double* c = sh + (key - key_lo);
+    const double t2 = t * t, t4 = t2 * t2;
+    {
+        const double p01 = c[1 * NS] * t + c[0], p23 = c[3 * NS] * t + c[2 * NS], p45 = c[5 * NS] * t + c[4 * NS], p67 = c[7 * NS] * t + c[6 * NS];
+        N = (p67 * t2 + p45) * t4 + (p23 * t2 + p01);
+    }
+    if (field) {
+        const double* d = c + (RT_DEG + 1) * NS;
+        const double p01 = d[1 * NS] * t + d[0], p23 = d[3 * NS] * t + d[2 * NS], p45 = d[5 * NS] * t + d[4 * NS], p67 = d[7 * NS] * t + d[6 * NS];
+        g = (p67 * t2 + p45) * t4 + (p23 * t2 + p01);
+    }
+}
+#endif
