@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-samples", type=int, nargs=2, default=None, help="two target counts for the oracle timing")
     ap.add_argument("--deterministic", action="store_true", help="PCE_FLAG_DETERMINISTIC: bit-reproducible gather (no fp64 atomics)")
+    ap.add_argument("--fig3d", action="store_true",
+                    help="the paper's timing workload (PAPER.md:325, Fig. 3d): induced-charge solve of FCC arrays vs total bead count; "
+                         "prints its own JSON line and exits")
     ap.add_argument("--bd", type=int, default=0, metavar="STEPS",
                     help="also run STEPS Brownian-dynamics steps on the device (solve + forces + pce_bd_step; config 3: 100, dt = 1e-4 a^2)")
     return ap.parse_args()
@@ -456,8 +459,43 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_fig3d(args):
+    """Time per induced-charge solve of FCC arrays of ideally polarizable spheres in a uniform field, no ions (the shape of the
+    paper's Fig. 3d, PAPER.md:325-327: N_b = 8 ... 512 bodies x N = 42 ... 2562 beads, spectral-Ewald tolerance 1e-3, GTX 1080;
+    here 4 m^3 bodies, reading B9), at the paper's tolerance and at this build's parity settings."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    import workloads as wl
+    pce.build()
+    rows = []
+    for m, subdiv in ((1, 3), (2, 3), (3, 3), (4, 3), (5, 3), (2, 4), (3, 4), (4, 4)):
+        w = wl.fcc_array(m, subdiv)
+        for tol, tol_solver in ((1e-3, 1e-3), (1e-10, 1e-12)):
+            ctx = pce.context_for(w, tol=tol, tol_solver=tol_solver)
+            x, y, z, Q, qi = pce.upload(w)
+            ctx.set_system(w.body_offset, x, y, z)
+            ts, its = [], []
+            for rep in range(4):
+                torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                ctx.set_positions(x, y, z)
+                q, Phi, si = ctx.solve(Q, qi, w.E0, allow_noconv=True)
+                b.record()
+                torch.cuda.synchronize()
+                if rep:
+                    ts.append(a.elapsed_time(b)); its.append(si["iters"])
+            rows.append({"bodies": w.N_body, "beads_per_body": w.N_bead // w.N_body, "N_T": w.N_bead, "grid": int(w.Ng[0]),
+                         "P": int(ctx.params.P), "ewald_tol": tol, "solver_tol": tol_solver, "iters": int(np.median(its)),
+                         "ms_per_solve": float(np.median(ts)), "converged": bool(si["converged"]), "fft_mode": ctx.info()["fft_mode"]})
+            ctx.close()
+    print(json.dumps({"fig3d": rows, "what": "ms per time step = cell lists + caches + induced-charge solve (cold start), FCC arrays, phi = 0.2, E0 = (0,0,1)"}))
+
+
 def main():
     args = parse()
+    if args.fig3d:
+        return run_fig3d(args)
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
     local_rank = int(os.environ.get("LOCAL_RANK", 0))

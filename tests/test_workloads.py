@@ -88,3 +88,22 @@ def test_fiber_generator():
     assert wi.N_ion == 50 and abs(wi.q_ion.sum()) < 1e-12
     dmin, _ = cKDTree(wi.x[:wi.N_bead]).query(wi.x[wi.N_bead:], k=1)
     assert dmin.min() >= 2.5 * wi.a
+
+
+def test_fcc_array_generator():
+    """FCC arrays of the paper's timing workload: 4 m^3 spheres, 12 nearest neighbours at a / sqrt 2 of the
+    conventional cell, the requested volume fraction, no overlaps."""
+    import numpy as np
+    from scipy.spatial import cKDTree
+    import workloads as wl
+    w = wl.fcc_array(2, subdiv=2, phi=0.3)
+    assert w.N_body == 32 and w.N_bead == 32 * 162 and w.N_ion == 0
+    c = w.meta["centres"]
+    L = float(w.L[0])
+    assert np.isclose(w.N_body * 4.0 / 3.0 * np.pi / L ** 3, 0.3)
+    pairs = cKDTree(c, boxsize=L).query_pairs((L / 2) / np.sqrt(2) * 1.001, output_type="ndarray")
+    assert len(pairs) == 32 * 12 // 2                      # every site has 12 nearest neighbours
+    d = c[pairs[:, 0]] - c[pairs[:, 1]]
+    d -= L * np.round(d / L)
+    assert np.allclose(np.linalg.norm(d, axis=1), (L / 2) / np.sqrt(2)) and (L / 2) / np.sqrt(2) > 2 + 2 * w.a
+    assert w.Ng[0] & (w.Ng[0] - 1) == 0 and L / w.Ng[0] <= 2.3 * w.a

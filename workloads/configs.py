@@ -145,6 +145,25 @@ def config4(seed=BASE_SEED + 4, subdiv=3, nside=4, spacing=4.0, n_ion=100000, Ng
                centres=centres)
 
 
+def fcc_array(m=2, subdiv=3, phi=0.2, Ng=None, h_over_a=2.3):
+    """FCC array of 4 m^3 ideally polarizable spheres (m conventional cells per dimension) in a uniform field, no ions: the
+    shape of the paper's only timing workload (Fig. 3d; reading B9: the paper counts N_b = 8 ... 512 bodies, an FCC
+    array in a periodic cube holds 4 m^3).  Sphere radius 1, volume fraction phi; mesh spacing at most h_over_a bead radii with N_g the next
+    power of two."""
+    mesh = geo.icosphere(subdiv)
+    a = geo.bead_radius(mesh)
+    cell = (4.0 * (4.0 / 3.0) * np.pi / phi) ** (1.0 / 3.0)   # 4 spheres per conventional cell
+    L = m * cell
+    basis = np.array([[0, 0, 0], [0, 0.5, 0.5], [0.5, 0, 0.5], [0.5, 0.5, 0]]) + 0.25
+    centres = np.array([(np.array([i, j, k]) + b) * cell for i in range(m) for j in range(m) for k in range(m) for b in basis])
+    beads = np.concatenate([mesh + c for c in centres])
+    off = np.arange(len(centres) + 1) * len(mesh)
+    if Ng is None:
+        Ng = int(2 ** np.ceil(np.log2(L / (h_over_a * a))))
+    return _mk(f"fcc_{len(centres)}x{len(mesh)}", beads, off, np.zeros(len(centres)), np.zeros((0, 3)), [], [0, 0, 1.0], L, Ng, a,
+               centres=centres, phi=phi)
+
+
 def config5(seed=BASE_SEED + 5, n_body=500, n_bead=1000, n_ion=1000000, phi=0.1, Ng=512, aspect=4.0):
     """n_body rigid prolate spheroids (1,1,aspect) at volume fraction phi with
     uniformly random orientations plus +-1 ions, E0 = (0.3,0,0)
