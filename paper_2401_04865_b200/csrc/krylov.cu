@@ -412,7 +412,7 @@ static int enqueue_iteration(pce_ctx* c)
     {
         PassTimer t(c, PASS_KRYLOV);
         k_pupdate<<<pupdate_blocks(c), 256, 0, c->st>>>(n, c->cg_g, pc ? c->cg_z : nullptr, c->pc_mean, c->body_of, c->bead.inv, c->wbead.inv,
-                                                        c->cg_p, c->bead.qs, c->use_cols ? c->wbead.qs_cols : c->wbead.qs, c->use_cols ? 16 : 1, c->cg_part, c->cg_state);
+                                                        c->cg_p, c->bead.qs, c->use_cols ? c->wbead.qs_cols : c->wbead.qs, c->use_cols ? HITREC_Q_STRIDE : 1, c->cg_part, c->cg_state);
         c->launches++;
     }
     rc = op_matvec_bead_sorted(c);

@@ -414,7 +414,7 @@ static int apply_operator(pce_ctx* c, Bins& sr, Bins& sw, Bins& tr, Bins& tw, bo
     {
         PassTimer t(c, PASS_OTHER);
         if ((rc = gather_by_perm(c, sr.n, sr.perm, q, sr.qs))) return rc;
-        if ((rc = gather_by_perm(c, sw.n, sw.perm, q, c->use_cols ? sw.qs_cols : sw.qs, c->use_cols ? 16 : 1))) return rc;
+        if ((rc = gather_by_perm(c, sw.n, sw.perm, q, c->use_cols ? sw.qs_cols : sw.qs, c->use_cols ? HITREC_Q_STRIDE : 1))) return rc;
         if ((rc = sum_vector(c, q, sr.n, c->scal))) return rc;
     }
     if (use_csr) rc = real_csr_spmv(c, sr, c->w_real);                                      // step 1 (cached), eq. 20-21

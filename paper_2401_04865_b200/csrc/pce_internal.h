@@ -13,14 +13,16 @@
 
 #define PCE_PI 3.14159265358979323846
 
-// 128-byte hit record of one particle for the cached-list spread / gather (wave_cols.cu): per dimension the coefficients
-// (c0, e1, e8, 1/e8) of the exp-free window recurrence, the first support index per dimension, and the particle's charge
+// 64-byte hit record of one particle for the cached-list spread / gather (wave_cols.cu): per dimension the two coefficients
+// (c_m, e1) of the exp-free window recurrence -- c_m = exp(-aw u0 (u0 + 2 (phi - 8))), the weight factor at support index
+// phi - 8, and e1 = exp(-2 aw u0) --, the first support index per dimension (int16: meshes up to 32767) and the charge
 struct alignas(16) HitRec {
-    double4 cf[3];
-    int4 s0;
-    double pad, q;
+    double2 cf[3];
+    short s0[3], pad;
+    double q;
 };
-static_assert(sizeof(HitRec) == 128, "hit records are 128 bytes");
+static_assert(sizeof(HitRec) == 64, "hit records are 64 bytes");
+constexpr int HITREC_Q_STRIDE = sizeof(HitRec) / sizeof(double);  // doubles between the charges of consecutive records
 
 // ---------------------------------------------------------------- binning
 // A counting-sort binning of a particle subset into a Cartesian cell grid
@@ -60,7 +62,7 @@ struct Bins {
     int2* items = nullptr;        // [col_item_cap] (brick, chunk)
     double* col_scratch = nullptr;  // [col_item_cap][512] partial bricks of split bricks
     int* col_arrive = nullptr;    // [ncell] arrival counters of split bricks
-    double* qs_cols = nullptr;    // &hrec[0].q: charges are written into the records (stride 16 doubles)
+    double* qs_cols = nullptr;    // &hrec[0].q: charges are written into the records (stride HITREC_Q_STRIDE doubles)
     int col_chunk = 0, n_items = 0;
     // deterministic gather (PCE_FLAG_DETERMINISTIC): pair numbering per brick, per-particle pair lists
     int* pair_start = nullptr;    // [ncell + 1]

@@ -3,7 +3,7 @@
 //
 // Positions are frozen for the ~30 operator applications of a Krylov solve, so everything that depends on
 // positions only is built once per pce_set_positions:
-//   * per particle a 128-byte hit record: first support index per dimension and the coefficients of the exp-free window
+//   * per particle a 64-byte hit record: first support index per dimension and the coefficients of the exp-free window
 //     recurrence (see wave_bricks.cu), plus the particle's charge (rewritten per application);
 //   * per brick COLUMN (bx, by) the list of particles whose (x, y) support meets the column, ordered by the first support
 //     plane z_k (counting sort on the key (column, z_k), ties by particle slot: deterministic).  The hits of brick
@@ -26,7 +26,7 @@ constexpr int CW = 4;           // warps per CTA
 constexpr int NTAB = 48 + 48;   // Gt[r + 8] = exp(-aw r^2), Ht[r + 8] = exp(-aw (2r + 1)), r = -8..39
 constexpr int STRIDE_PSI = 26;  // doubles per hit in the weight table: 3 x 8 + 2 pad
 constexpr int STRIDE_FLD = 50;  // with the field: 3 x (8 w + 8 w u) + 2 pad
-constexpr int REC_BYTES = 128;
+constexpr int REC_BYTES = 64;
 
 __device__ __forceinline__ int wrap_once(int d, int n) { if (d < 0) d += n; if (d >= n) d -= n; return d; }
 
@@ -49,8 +49,8 @@ struct ColGeom {
 };
 
 // ---------------------------------------------------------------- once per position update
-// hit record of sorted particle i: window-recurrence coefficients (c0, e1, e8, 1/e8) per dimension, first support index per
-// dimension, charge (filled per application), and u0 = s0 - x/h (field gather only) in a second array
+// hit record of sorted particle i: window-recurrence coefficients (c_m, e1) per dimension, first support index per dimension,
+// charge (filled per application), and u0 = s0 - x/h (field gather only) in a second array
 __global__ void __launch_bounds__(256)
 k_hit_records(int n, WaveConst wc, const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
               HitRec* __restrict__ rec, double4* __restrict__ u0o)
@@ -69,10 +69,10 @@ k_hit_records(int n, WaveConst wc, const double* __restrict__ xs, const double* 
         const double u0 = (double)s0 - xd; // in (-P/2, -P/2 + 1]
         const int phi = (-s0) & (BR - 1);
         sv[d] = s0; uv[d] = u0;
-        r.cf[d] = make_double4(exp(-wc.aw * u0 * (u0 + 2.0 * phi)), exp(-2.0 * wc.aw * u0), exp(-16.0 * wc.aw * u0), exp(16.0 * wc.aw * u0));
+        r.cf[d] = make_double2(exp(-wc.aw * u0 * (u0 + 2.0 * (phi - BR))), exp(-2.0 * wc.aw * u0));
     }
-    r.s0 = make_int4(sv[0], sv[1], sv[2], 0);
-    r.pad = 0.0; r.q = 0.0;
+    r.s0[0] = (short)sv[0]; r.s0[1] = (short)sv[1]; r.s0[2] = (short)sv[2]; r.pad = 0;
+    r.q = 0.0;
     rec[i] = r;
     u0o[i] = make_double4(uv[0], uv[1], uv[2], 0.0);
 }
@@ -84,7 +84,7 @@ k_col_keys(int n, ColGeom g, const HitRec* __restrict__ rec, int* __restrict__ c
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int4 s0 = rec[i].s0;
+    const int4 s0 = make_int4(rec[i].s0[0], rec[i].s0[1], rec[i].s0[2], 0);
     const int fx = s0.x >> 3, lx = (s0.x + g.P - 1) >> 3, fy = s0.y >> 3, ly = (s0.y + g.P - 1) >> 3;  // >> 3: floor for negatives too
     const int zk = s0.z < 0 ? s0.z + g.Nz : s0.z;
     for (int iy = fy; iy <= ly; ++iy) {
@@ -245,16 +245,16 @@ __device__ __forceinline__ int hit_slot(const Item& it, const int* __restrict__ 
     return ent[h < it.n0 ? it.a0 + h : it.a1 + (h - it.n0)];
 }
 
-// stream the records of 32 hits (slot p per lane, -1: none) into the warp's buffer: instruction k moves records 4k..4k+3 whole
-// (8 lanes x 16 bytes each), chunk c of record r lands at r*128 + ((c ^ (r & 7)) * 16): conflict-free 16-byte reads per lane later
+// stream the records of 32 hits (slot p per lane, -1: none) into the warp's buffer: instruction k moves records 8k..8k+7 whole
+// (4 lanes x 16 bytes each), chunk c of record r lands at r*64 + ((c ^ ((r >> 1) & 3)) * 16): conflict-free 16-byte reads per lane later
 __device__ __forceinline__ void prefetch_records(unsigned char* __restrict__ rbuf, const HitRec* __restrict__ rec, int p, int lane)
 {
-    const int c = lane & 7;
+    const int c = lane & 3;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        const int r = 4 * k + (lane >> 3);
+    for (int k = 0; k < 4; ++k) {
+        const int r = 8 * k + (lane >> 2);
         const int pr = __shfl_sync(0xffffffffu, p, r);
-        if (pr >= 0) cp_async16(rbuf + r * REC_BYTES + ((c ^ (r & 7)) << 4), reinterpret_cast<const unsigned char*>(rec + pr) + (c << 4));
+        if (pr >= 0) cp_async16(rbuf + r * REC_BYTES + ((c ^ ((r >> 1) & 3)) << 4), reinterpret_cast<const unsigned char*>(rec + pr) + (c << 4));
     }
     cp_async_commit();
 }
@@ -268,24 +268,25 @@ __device__ __forceinline__ double4 ld_u0(const double4* __restrict__ u0g, int p)
 template <class T>
 __device__ __forceinline__ T rec_chunk(const unsigned char* rbuf, int r, int c)
 {
-    return *reinterpret_cast<const T*>(rbuf + r * REC_BYTES + ((c ^ (r & 7)) << 4));
+    return *reinterpret_cast<const T*>(rbuf + r * REC_BYTES + ((c ^ ((r >> 1) & 3)) << 4));
 }
 
 // the 8 brick-local window weights of one hit in one dimension (0 outside the support) and, with FIELD, the weights times
-// u = (mesh index - x/h); returns the mask of live brick-local points.  cf = (c0, e1, e8, 1/e8), tab = [Gt | Ht].
+// u = (mesh index - x/h); returns the mask of live brick-local points.  cf = (c_m, e1): weight factor at support index phi - 8
+// and exp(-2 aw u0); tab = [Gt | Ht].
 template <bool FIELD>
-__device__ __forceinline__ unsigned brick_weights(int P, const double* __restrict__ tab, int b0, int ng, int s0, const double4 cf, double u0,
+__device__ __forceinline__ unsigned brick_weights(int P, const double* __restrict__ tab, int b0, int ng, int s0, const double2 cf, double u0,
                                                   double scale, double* __restrict__ w)
 {
     int r0 = b0 - s0;                   // support index of brick-local point 0, brought into -7 .. P-1
     if (r0 >= P) r0 -= ng;
     if (r0 < -7) r0 += ng;
     const int phi = (-s0) & (BR - 1);
-    const int m = (r0 - phi) >> 3;      // -1 .. 3: r0 = phi + 8 m
-    double pm = (m < 0) ? cf.w : 1.0;   // e8^m
-    if (m >= 1) pm = cf.z;
-    if (m >= 2) pm *= cf.z;
-    if (m >= 3) pm *= cf.z;
+    const int m1 = ((r0 - phi) >> 3) + 1;  // 0 .. 4: r0 = phi - 8 + 8 m1
+    const double e2 = cf.y * cf.y, e4 = e2 * e2, e8 = e4 * e4, e16 = e8 * e8;
+    double pm = (m1 & 1) ? e8 : 1.0;       // e8^m1
+    if (m1 & 2) pm *= e16;
+    if (m1 & 4) pm = e16 * e16;
     double pw = cf.x * pm * tab[r0 + 8] * scale;
     double t = cf.y * tab[48 + r0 + 8];
     const double g2 = tab[9] * tab[9];  // exp(-2 aw)
@@ -325,15 +326,16 @@ __device__ __forceinline__ void batch_weights(const WaveConst& wc, const double*
 {
     unsigned zmask = 0;
     if (lane < nh) {
-        const int4 s0 = rec_chunk<int4>(s.rec, lane, 6);
-        const double q = use_q ? rec_chunk<double2>(s.rec, lane, 7).y : 1.0;
+        const double2 sq = rec_chunk<double2>(s.rec, lane, 3);   // (s0 as 3 x int16, charge)
+        const int shi = __double2hiint(sq.x), slo = __double2loint(sq.x);
+        const int4 s0 = make_int4((int)(short)(slo & 0xffff), slo >> 16, (int)(short)(shi & 0xffff), 0);
+        const double q = use_q ? sq.y : 1.0;
         double* w = s.wt + lane * STRIDE;
         const int sv[3] = {s0.x, s0.y, s0.z};
         const double uv[3] = {u0v.x, u0v.y, u0v.z};
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const double2 c01 = rec_chunk<double2>(s.rec, lane, 2 * d), c23 = rec_chunk<double2>(s.rec, lane, 2 * d + 1);
-            const unsigned lv = brick_weights<FIELD>(wc.P, tab, it.b0[d], wc.Ng[d], sv[d], make_double4(c01.x, c01.y, c23.x, c23.y), uv[d],
+            const unsigned lv = brick_weights<FIELD>(wc.P, tab, it.b0[d], wc.Ng[d], sv[d], rec_chunk<double2>(s.rec, lane, d), uv[d],
                                                      d == 2 ? q : 1.0, w + DW * d);
             if (d == 2) zmask = lv;
         }
@@ -353,7 +355,7 @@ __device__ __forceinline__ void batch_weights(const WaveConst& wc, const double*
 // H_z[y][x] = sum_h (wy_h[y] q_h wz_h[z]) wx_h[x] per plane z of the brick, four hits per fp64 mma, planes dead for the whole
 // group skipped.  A brick split into several items (crowded bricks on small meshes) is combined deterministically: every item
 // stores its partial brick in scratch, the item that arrives last adds them in item order and writes the mesh.
-__global__ void __launch_bounds__(CW * 32, 5)
+__global__ void __launch_bounds__(CW * 32, 6)
 k_spread_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const int* __restrict__ ent, const int2* __restrict__ items,
               int n_items, const int* __restrict__ item_start, const HitRec* __restrict__ rec, double* __restrict__ grid,
               double* __restrict__ scratch, int* __restrict__ arrive, int* __restrict__ work_ctr, const int* __restrict__ skip)
@@ -455,7 +457,7 @@ k_spread_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const 
 // operand), U[h][x] += wz_h[z] T_z[h][x], psi_h += sum_x wx_h[x] U[h][x]; one atomicAdd per hit, item and quantity.  With the
 // field the window-gradient sums (reading A3) reuse T_z with wz u_z and wx u_x and need a second contraction with wy u_y.
 template <bool FIELD>
-__global__ void __launch_bounds__(CW * 32, FIELD ? 3 : 5)
+__global__ void __launch_bounds__(CW * 32, FIELD ? 3 : 6)
 k_gather_cols(WaveConst wc, ColGeom g, const int* __restrict__ key_start, const int* __restrict__ ent, const int2* __restrict__ items,
               int n_items, const int* __restrict__ item_start, const HitRec* __restrict__ rec, const double4* __restrict__ u0g,
               const double* __restrict__ grid,
@@ -633,7 +635,7 @@ k_inv_count(int n, int P, const HitRec* __restrict__ rec, int* __restrict__ inv_
     if (i > n) return;
     int v = 0;
     if (i < n) {
-        const int4 s0 = rec[i].s0;
+        const int4 s0 = make_int4(rec[i].s0[0], rec[i].s0[1], rec[i].s0[2], 0);
         int f, cx, cy, cz;
         brick_span(s0.x, P, f, cx); brick_span(s0.y, P, f, cy); brick_span(s0.z, P, f, cz);
         v = cx * cy * cz;
@@ -656,7 +658,7 @@ k_inv_fill(int nbrick, ColGeom g, const int* __restrict__ key_start, const int* 
     const int base = pair_start[b];
     for (int h = lane; h < n0 + n1; h += 32) {
         const int p = ent[h < n0 ? a0 + h : a1 + (h - n0)];
-        const int4 s0 = rec[p].s0;
+        const int4 s0 = make_int4(rec[p].s0[0], rec[p].s0[1], rec[p].s0[2], 0);
         int fx, fy, fz, cx, cy, cz;
         brick_span(s0.x, g.P, fx, cx); brick_span(s0.y, g.P, fy, cy); brick_span(s0.z, g.P, fz, cz);
         int dx = (bx - fx) % g.nbx, dy = (by - fy) % g.nby, dz = (bz - fz) % g.nbz;
@@ -753,7 +755,7 @@ int wave_cols_alloc(pce_ctx* c, Bins& b)
         c->bytes += (long long)((nbrick + 1 + n + 1) * 4);
     }
     b.nkeys = (long long)nkeys;
-    b.qs_cols = reinterpret_cast<double*>(b.hrec) + 15;  // the charge sits in the last 8 bytes of every 128-byte record
+    b.qs_cols = reinterpret_cast<double*>(b.hrec) + (HITREC_Q_STRIDE - 1);  // the charge sits in the last 8 bytes of every record
     return PCE_OK;
 }
 
