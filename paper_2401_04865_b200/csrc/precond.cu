@@ -249,7 +249,7 @@ k_pc_final(const PcBody* __restrict__ bodies, const double* __restrict__ work, c
 // ---------------------------------------------------------------- apply: z_raw = B r (rows of one body per CTA)
 struct PcRows { int j0, n, row0; int pad; long long boff; };  // CTA -> body, first row
 
-constexpr int PC_ROWS = 32;  // rows per CTA (4 per warp)
+constexpr int PC_ROWS = 64;  // rows per CTA (8 per warp: one shared-memory read of the residual serves 8 rows)
 
 __device__ __forceinline__ double bf16_lo(unsigned w) { return (double)__uint_as_float(w << 16); }
 __device__ __forceinline__ double bf16_hi(unsigned w) { return (double)__uint_as_float(w & 0xffff0000u); }
