@@ -169,3 +169,29 @@ def test_deterministic_flag_gives_bit_identical_results():
     w2 = wl.tiny_random(seed=3, n_body=1, n_ion=10, L=6.0, Ng=36)
     with pytest.raises(pce.PceError):
         pce.context_for(w2, deterministic=True)
+
+
+def test_own_fft_passes_on_a_mesh_with_fewer_planes_than_rows():
+    """FFT mode 2 (own (x, y) passes + fused z pass) on a 128 x 128 x 64 mesh in a flat box: the plane pipeline of fftxy.cu with
+    N_z != N_x, against the oracle and against the cuFFT 3-D arrangement."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.tiny_random(seed=41, n_body=2, n_ion=60, L=6.0, Ng=32)
+    w.L = np.array([12.0, 12.0, 6.0])
+    w.Ng = np.array([128, 128, 64])
+    rng = np.random.default_rng(2)
+    q = rng.normal(size=w.N)
+    q -= q.mean()
+    psi_o, E_o = orc.ewald_eval(w.x, q, w.L, w.a)
+    res = {}
+    for fused in (True, False):
+        ctx = pce.context_for(w, fused_z=fused)
+        assert ctx.info()["fft_mode"] == (2 if fused else 0)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        out = ctx.evaluate(torch.from_numpy(q).cuda())
+        res[fused] = (out[0].cpu().numpy(), _E(out))
+        assert rel(res[fused][0], psi_o) < 1e-9 and rel(res[fused][1], E_o) < 1e-9
+        ctx.close()
+    assert rel(res[True][0], res[False][0]) < 1e-12
