@@ -195,3 +195,33 @@ def test_own_fft_passes_on_a_mesh_with_fewer_planes_than_rows():
         assert rel(res[fused][0], psi_o) < 1e-9 and rel(res[fused][1], E_o) < 1e-9
         ctx.close()
     assert rel(res[True][0], res[False][0]) < 1e-12
+
+
+@pytest.mark.parametrize("ng", [256, 512])
+def test_large_mesh_passes_against_the_oracle_on_full_vectors(ng):
+    """The 256- and 512-point instances of the own FFT passes and of the fused z pass pinned to the oracle on EVERY particle (the
+    oracle's cost depends on the particle count only, so a small system on a large mesh is cheap to check): potentials, fields,
+    induced charges, torques."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.tiny_random(seed=50 + ng, n_body=2, n_ion=50, L=6.0, Ng=ng, neutral=False)
+    # Ewald tolerance 1e-11 (P = 22): the torque of a 12-bead icosahedron is a small difference of r x f terms, so the relative
+    # torque error is the relative force error times that cancellation (about 10 here)
+    ctx = pce.context_for(w, tol=1e-11)
+    assert ctx.info()["fft_mode"] == 2
+    x, y, z, Q, qi = pce.upload(w)
+    ctx.set_system(w.body_offset, x, y, z)
+    rng = np.random.default_rng(ng)
+    qv = rng.normal(size=w.N)
+    out = ctx.evaluate(torch.from_numpy(qv).cuda())
+    psi_o, E_o = orc.ewald_eval(w.x, qv, w.L, w.a)
+    assert rel(out[0].cpu().numpy(), psi_o) < 1e-9 and rel(_E(out), E_o) < 1e-9
+    q, Phi, info = ctx.solve(Q, qi, w.E0)
+    f = ctx.forces(q, w.E0)
+    qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+    oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, Phi_body=Phio)
+    assert info["converged"] and rel(q.cpu().numpy(), qo) < 1e-9
+    assert rel(f["f"].cpu().numpy(), oo["f"]) < 1e-8
+    assert body_vector_error(f["T"].cpu().numpy(), oo["T"], oo["f"])[0] < 1e-8
+    ctx.close()
