@@ -322,6 +322,8 @@ int fftxy_init(pce_ctx* c)
     PCE_CUDA(c, cudaMalloc(&c->xytw, tw.size() * sizeof(double2)));
     PCE_CUDA(c, cudaMemcpy(c->xytw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice));
     PCE_CUDA(c, cudaMalloc(&c->xy_ctr, ((size_t)c->p.Ng[2] + 1) * sizeof(int)));
+    // threads per CTA of the forward / inverse kernel: 256 (measured best at 512^3: 0.79 / 0.89 ms; 128 threads 1.00 / 1.15 ms,
+    // 512 threads 0.83 / 0.93 ms); the environment variables select the other instantiations for tuning on other meshes
     const char* ef = getenv("PCE_FFTXY_NT_F");
     const char* ei = getenv("PCE_FFTXY_NT_I");
     c->xy_nt[0] = (ef && (atoi(ef) == 128 || atoi(ef) == 512)) ? atoi(ef) : 256;
