@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-samples", type=int, nargs=2, default=None, help="two target counts for the oracle timing")
+    ap.add_argument("--P-matvec", type=int, default=0, help="narrower window for the solver matvec (pce_params.P_matvec; default: P)")
     ap.add_argument("--deterministic", action="store_true", help="PCE_FLAG_DETERMINISTIC: bit-reproducible gather (no fp64 atomics)")
     ap.add_argument("--fig3d", action="store_true",
                     help="the paper's timing workload (PAPER.md:325, Fig. 3d): induced-charge solve of FCC arrays vs total bead count; "
@@ -75,7 +76,7 @@ def config_dict(w, args):
     prm = pce.suggest_params(w.L, w.Ng, w.a, args.tol, args.P)
     grid_bytes = 8 * int(np.prod(w.Ng))
     return {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "N_body": w.N_body, "grid": [int(g) for g in w.Ng],
-            "P": int(prm.P), "xi": prm.xi, "rc": prm.rc, "ewald_tol": args.tol, "solver_tol": args.tol_solver,
+            "P": int(prm.P), "P_matvec": int(args.P_matvec or prm.P_matvec), "xi": prm.xi, "rc": prm.rc, "ewald_tol": args.tol, "solver_tol": args.tol_solver,
             "l2": "flushed between timed steps" if grid_bytes < 256 << 20 else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
             "multi_gpu": "replicas only"}
 
@@ -235,7 +236,7 @@ def run_ours(args, rank, world, local_rank):
     if dist:
         dist.barrier()
     w = make_workload(args.config, rank)
-    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, deterministic=args.deterministic)
+    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, deterministic=args.deterministic, P_matvec=args.P_matvec)
     x, y, z, Q, qi = pce.upload(w)
     ctx.set_system(w.body_offset, x, y, z)
     info = ctx.info()
@@ -380,6 +381,7 @@ def run_ours(args, rank, world, local_rank):
 
     dfma_tf, dmma_tf = pce.measure_fp64_peaks()  # live, on this device (csrc/peaks.cu)
     P3 = float(ctx.params.P) ** 3
+    P3b = float(info["P_matvec"]) ** 3   # the solver matvec spreads / gathers with its own, narrower window (pce.h: P_matvec)
 
     def rf(ms_total, launches_, bytes_per_launch, fma_per_launch=None):
         """HBM roofline of a pass; passes bound by fp64 arithmetic (fma_per_launch given: useful window updates, 2 flop each)
@@ -407,8 +409,8 @@ def run_ours(args, rank, world, local_rank):
         flavours["m1_bead_matvec"].update({"algorithmic_bytes": m1_bytes, "hbm_ceiling_per_s": hbm_peak * 1e9 / m1_bytes,
                                            "frac_of_hbm_ceiling": flavours["m1_bead_matvec"]["per_s"] * m1_bytes / (hbm_peak * 1e9)})
     passes = {
-        "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3, w.N_bead * P3),
-        "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead, w.N_bead * P3),
+        "spread_bead": rf(acc["bead_spread"], nm1, 32 * w.N_bead + 8 * Ng3, w.N_bead * P3b),
+        "gather_bead": rf(acc["bead_gather"], nm1, 8 * Ng3 + 40 * w.N_bead, w.N_bead * P3b),
         "real_bead_csr": rf(acc["bead_real"], nm1, 12 * info["nnz_near"] + 20 * w.N_bead),
         "scale": rf(acc["scale"], npairs, 32 * Nk),
         fft_keys[0]: rf(acc["fft"], npairs, 8 * Ng3 + 16 * Nk),

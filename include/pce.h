@@ -81,6 +81,14 @@ typedef struct {
     double tol_solver;  /* relative residual at which the Krylov solve stops */
     int    max_iter;    /* iteration cap of the Krylov solve */
     int    flags;       /* 0, or PCE_FLAG_* ORed */
+    int    P_matvec;    /* support points per dimension of the SOLVER's bead-only matvec (pce_matvec, the Krylov iterations);
+                           0 or P: the same window as everywhere (what pce_suggest_params sets).  The solver needs potentials
+                           only, and at equal P the potential is ~5-20x more accurate than the window-gradient field, so
+                           P - 2 keeps the induced charges within the tolerance (config 2: q error 5e-11 at P_matvec = 18,
+                           tol 1e-10) and makes the spread / gather of every iteration (P_matvec / P)^3 = 0.73x as expensive
+                           (config 5: step 184 -> 173 ms); the price is in ill-conditioned derived quantities -- the torque on
+                           two nearly touching spheres (config 2, d = 2.2: a difference 1e5 times smaller than its terms)
+                           moves from 7e-9 to 4e-8 relative.  Even, 4..P */
 } pce_params;
 
 typedef struct {
@@ -112,6 +120,7 @@ typedef struct {
     long long bytes_workspace;
     long long bytes_precond; /* storage of the block-Jacobi preconditioner (bf16 for many large bodies, else fp32; 0: off) */
     int n_precond_blocks;    /* bodies that own a dense preconditioner block */
+    int P_matvec;            /* support points per dimension of the solver's bead-only matvec */
     int fft_mode;            /* 0: cuFFT 3-D plans + scaling pass; 1: cuFFT 2-D per plane + fused z pass; 2: own (x, y) passes + fused z pass */
 } pce_info;
 
@@ -119,8 +128,8 @@ typedef struct {
  * s^2 = -ln tol; k_c = pi (Ng-1)/L; xi = k_c/(2s) (eq. 28);
  * r_c = s/xi + 2a (eq. 23; the +2a because eq. 20 decays like
  * erfc((r-2a) xi) for shells, reading A14); P even with
- * exp(-pi P/2) a factor ~500 below tol (eq. 32).  P_override > 0 fixes P.
- * Fills L, Ng, xi, rc, P, a, eps_f=1, tol_solver=1e-12, max_iter=500. */
+ * exp(-pi P/2) a factor ~500 below tol (eq. 32), P_matvec = P.  P_override > 0 fixes P.
+ * Fills L, Ng, xi, rc, P, P_matvec, a, eps_f=1, tol_solver=1e-12, max_iter=500. */
 int pce_suggest_params(const double L[3], const int Ng[3], double a, double tol,
                        int P_override, pce_params* out);
 

@@ -29,7 +29,7 @@ EXPORTS = (
 class PceParams(C.Structure):
     _fields_ = [("L", C.c_double * 3), ("Ng", C.c_int * 3), ("xi", C.c_double), ("rc", C.c_double), ("P", C.c_int),
                 ("a", C.c_double), ("eps_f", C.c_double), ("tol_solver", C.c_double), ("max_iter", C.c_int),
-                ("flags", C.c_int)]
+                ("flags", C.c_int), ("P_matvec", C.c_int)]
 
 
 class PceSolveInfo(C.Structure):
@@ -53,7 +53,7 @@ class PceTimings(C.Structure):
 class PceInfo(C.Structure):
     _fields_ = [("eta", C.c_double * 3), ("h", C.c_double * 3), ("ncell", C.c_int * 3), ("image_range", C.c_int * 3),
                 ("nnz_near", C.c_longlong), ("N", C.c_int), ("N_bead", C.c_int), ("N_body", C.c_int),
-                ("bytes_workspace", C.c_longlong), ("bytes_precond", C.c_longlong), ("n_precond_blocks", C.c_int), ("fft_mode", C.c_int)]
+                ("bytes_workspace", C.c_longlong), ("bytes_precond", C.c_longlong), ("n_precond_blocks", C.c_int), ("P_matvec", C.c_int), ("fft_mode", C.c_int)]
 
 
 class PceError(RuntimeError):
@@ -327,7 +327,7 @@ class Context:
         self._ck(self.lib.pce_get_info(self.h, C.byref(i)))
         return {"eta": list(i.eta), "h": list(i.h), "ncell": list(i.ncell), "image_range": list(i.image_range),
                 "nnz_near": i.nnz_near, "N": i.N, "N_bead": i.N_bead, "N_body": i.N_body, "bytes_workspace": i.bytes_workspace,
-                "bytes_precond": i.bytes_precond, "n_precond_blocks": i.n_precond_blocks, "fft_mode": i.fft_mode}
+                "bytes_precond": i.bytes_precond, "n_precond_blocks": i.n_precond_blocks, "P_matvec": i.P_matvec, "fft_mode": i.fft_mode}
 
     def launch_count(self):
         return int(self.lib.pce_launch_count(self.h))
@@ -339,11 +339,13 @@ PCE_FLAG_FIELD_IK = 4
 PCE_FLAG_DETERMINISTIC = 8
 
 
-def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None, precond=True, fused_z=True, field_ik=False, deterministic=False) -> Context:
+def context_for(workload, tol=1e-10, P=0, tol_solver=1e-12, max_iter=500, stream=None, precond=True, fused_z=True, field_ik=False, deterministic=False, P_matvec=0) -> Context:
     """Context with parameters suggested for a workloads.Workload."""
     p = suggest_params(workload.L, workload.Ng, workload.a, tol, P)
     p.flags = (0 if precond else PCE_FLAG_NO_PRECOND) | (0 if fused_z else PCE_FLAG_CUFFT_3D) | (PCE_FLAG_FIELD_IK if field_ik else 0) | (PCE_FLAG_DETERMINISTIC if deterministic else 0)
     p.eps_f = workload.eps_f
+    if P_matvec:
+        p.P_matvec = int(P_matvec)
     p.tol_solver = tol_solver
     p.max_iter = max_iter
     return Context(p, stream)

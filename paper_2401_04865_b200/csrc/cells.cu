@@ -238,7 +238,7 @@ int bins_alloc_tiles(pce_ctx* c, Bins& b, int n, int tile)
     // the same 1/h the mesh kernels use, so that floor(x/h) agrees bit for bit
     // bins are shifted by P/2 mod tile so that the mesh cells whose support meets a brick span the fewest bins
     for (int d = 0; d < 3; ++d) {
-        b.scale[d] = c->wk.inv_h[d]; b.imax[d] = c->p.Ng[d] - 1; b.div[d] = tile; b.shift[d] = (c->p.P / 2) % tile;
+        b.scale[d] = c->wk.inv_h[d]; b.imax[d] = c->p.Ng[d] - 1; b.div[d] = tile; b.shift[d] = (c->wk.P / 2) % tile;  // the active window (wave_select)
     }
     return PCE_OK;
 }

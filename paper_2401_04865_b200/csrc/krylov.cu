@@ -411,14 +411,14 @@ static int enqueue_iteration(pce_ctx* c)
     c->skip_flag = &c->cg_state->done;
     {
         PassTimer t(c, PASS_KRYLOV);
-        k_pupdate<<<pupdate_blocks(c), 256, 0, c->st>>>(n, c->cg_g, pc ? c->cg_z : nullptr, c->pc_mean, c->body_of, c->bead.inv, c->wbead.inv,
-                                                        c->cg_p, c->bead.qs, c->use_cols ? c->wbead.qs_cols : c->wbead.qs, c->use_cols ? HITREC_Q_STRIDE : 1, c->cg_part, c->cg_state);
+        k_pupdate<<<pupdate_blocks(c), 256, 0, c->st>>>(n, c->cg_g, pc ? c->cg_z : nullptr, c->pc_mean, c->body_of, c->bead.inv, c->wmv->inv,
+                                                        c->cg_p, c->bead.qs, c->use_cols ? c->wmv->qs_cols : c->wmv->qs, c->use_cols ? HITREC_Q_STRIDE : 1, c->cg_part, c->cg_state);
         c->launches++;
     }
     rc = op_matvec_bead_sorted(c);
     if (!rc) {
         PassTimer t(c, PASS_KRYLOV);
-        k_proj_dot<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->bead.inv, c->wbead.inv, c->w_real, c->w_wave, c->kconst, c->cg_p, c->cg_t, c->cg_ap,
+        k_proj_dot<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->bead.inv, c->wmv->inv, c->w_real, c->w_wave, c->kconst, c->cg_p, c->cg_t, c->cg_ap,
                                         c->cg_part, c->cg_state);
         k_cg_update<<<nb, BT, 0, c->st>>>(nb, c->body_off, c->cg_p, c->cg_ap, c->cg_t, c->cg_q, c->cg_g, c->cg_psi, c->cg_part, c->cg_state,
                                          c->cg_host_dev, pc ? 1 : 0);

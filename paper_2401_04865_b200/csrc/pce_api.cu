@@ -30,6 +30,7 @@ extern "C" int pce_suggest_params(const double L[3], const int Ng[3], double a, 
     std::memset(out, 0, sizeof(*out));
     for (int d = 0; d < 3; ++d) { out->L[d] = L[d]; out->Ng[d] = Ng[d]; }
     out->xi = xi; out->rc = rc; out->P = P; out->a = a; out->eps_f = 1.0;
+    out->P_matvec = P;  // the same window for the solver matvec (a narrower one is the caller's choice, pce.h)
     out->tol_solver = 1e-12; out->max_iter = 500; out->flags = 0;
     return PCE_OK;
 }
@@ -68,7 +69,7 @@ static void free_system(pce_ctx* c)
 {
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z); cudaFree(c->body_off); cudaFree(c->body_of);
     cudaFree(c->rx); cudaFree(c->ry); cudaFree(c->rz); cudaFree(c->X); cudaFree(c->Y); cudaFree(c->Z);
-    bins_free(c->all); bins_free(c->bead); bins_free(c->wall); bins_free(c->wbead);
+    bins_free(c->all); bins_free(c->bead); bins_free(c->wall); bins_free(c->wbead); bins_free(c->wbead_s);
     cudaFree(c->csr_ptr); cudaFree(c->csr_col); cudaFree(c->csr_val);
     cudaFree(c->w_real); cudaFree(c->w_wave); cudaFree(c->w_ex); cudaFree(c->w_ey); cudaFree(c->w_ez);
     cudaFree(c->w_kx); cudaFree(c->w_ky); cudaFree(c->w_kz);
@@ -98,7 +99,7 @@ extern "C" int pce_destroy(pce_ctx* c)
     free_system(c);
     krylov_free(c);
     if (c->have_plans) { cufftDestroy(c->planF); cufftDestroy(c->planB); }
-    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp); cudaFree(c->zshape); cudaFree(c->xytw); cudaFree(c->xy_ctr); cudaFree(c->gather_part);
+    cudaFree(c->fft_work); cudaFree(c->grid); cudaFree(c->gridk); cudaFree(c->gridk2); cudaFree(c->scal); cudaFree(c->sum_part); cudaFree(c->scan_tmp); cudaFree(c->work_ctr); cudaFree(c->rt_dev); cudaFree(c->ztw); cudaFree(c->zexp_set[0]); cudaFree(c->zexp_set[1]); cudaFree(c->zshape); cudaFree(c->xytw); cudaFree(c->xy_ctr); cudaFree(c->gather_part);
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return PCE_OK;
@@ -106,29 +107,49 @@ extern "C" int pce_destroy(pce_ctx* c)
 
 extern "C" const char* pce_last_error(const pce_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
 
+// wave-space constants of a window with P support points per dimension (eq. 25, 31: eta = h^2 xi^2 P / pi)
+static void wave_const_for(const pce_ctx* c, int P, WaveConst& w)
+{
+    const pce_params& p = c->p;
+    double cn2 = 1.0, h3 = 1.0, ntot = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        const double h = p.L[d] / p.Ng[d], eta = h * h * p.xi * p.xi * P / PCE_PI;
+        w.Ng[d] = p.Ng[d]; w.L[d] = p.L[d]; w.h[d] = h; w.inv_h[d] = 1.0 / h;
+        w.kfac[d] = 2.0 * PCE_PI / p.L[d];
+        w.gexp[d] = (1.0 - eta) / (4.0 * p.xi * p.xi);
+        w.grad_fac[d] = 4.0 * PCE_PI / (P * h);
+        cn2 *= 2.0 / (P * h * h);
+        h3 *= h;
+        ntot *= p.Ng[d];
+    }
+    w.Nxh = p.Ng[0] / 2 + 1;
+    w.P = P;
+    w.aw = 2.0 * PCE_PI / P;
+    w.a = p.a;
+    w.scale_norm = cn2 * h3 / (p.eps_f * ntot);
+    for (int r = 0; r < 32; ++r) w.G[r] = std::exp(-w.aw * r * r);
+}
+
+// the window of the next wave passes: 0 = P (evaluations with fields, right-hand side), 1 = P_matvec (solver matvec)
+void wave_select(pce_ctx* c, int which)
+{
+    c->wk = c->wset[which];
+    c->zexp = c->zexp_set[which];
+}
+
 static int create_impl(pce_ctx* c)
 {
     const pce_params& p = c->p;
     c->V = p.L[0] * p.L[1] * p.L[2];
-    WaveConst& w = c->wk;
-    double cn2 = 1.0, h3 = 1.0, ntot = 1.0;
     for (int d = 0; d < 3; ++d) {
         c->h[d] = p.L[d] / p.Ng[d];
         c->eta[d] = c->h[d] * c->h[d] * p.xi * p.xi * p.P / PCE_PI;  // eq. 31
-        w.Ng[d] = p.Ng[d]; w.L[d] = p.L[d]; w.h[d] = c->h[d]; w.inv_h[d] = 1.0 / c->h[d];
-        w.kfac[d] = 2.0 * PCE_PI / p.L[d];
-        w.gexp[d] = (1.0 - c->eta[d]) / (4.0 * p.xi * p.xi);
-        w.grad_fac[d] = 4.0 * PCE_PI / (p.P * c->h[d]);
-        cn2 *= 2.0 / (p.P * c->h[d] * c->h[d]);
-        h3 *= c->h[d];
-        ntot *= p.Ng[d];
     }
-    w.Nxh = p.Ng[0] / 2 + 1;
-    w.P = p.P;
-    w.aw = 2.0 * PCE_PI / p.P;
-    w.a = p.a;
-    w.scale_norm = cn2 * h3 / (p.eps_f * ntot);
-    for (int r = 0; r < 32; ++r) w.G[r] = std::exp(-w.aw * r * r);
+    c->P_mv = (p.P_matvec >= 4 && p.P_matvec < p.P) ? p.P_matvec : p.P;
+    wave_const_for(c, p.P, c->wset[0]);
+    wave_const_for(c, c->P_mv, c->wset[1]);
+    c->wk = c->wset[0];
+    WaveConst& w = c->wk;
     RealConst& r = c->rk;
     r.a = p.a; r.xi = p.xi; r.two_a = 2.0 * p.a; r.inv_eps = 1.0 / p.eps_f;
     r.c64 = 1.0 / (64.0 * PCE_PI * p.a * p.a * p.xi * p.xi);
@@ -201,7 +222,8 @@ extern "C" int pce_create(const pce_params* p, void* stream, pce_ctx** out)
     bool ok = p->xi > 0 && p->rc > 0 && p->a > 0 && p->eps_f > 0 && p->P >= 4 && p->P <= 32 && (p->P % 2 == 0) && p->max_iter > 0 &&
               p->tol_solver > 0;
     for (int d = 0; d < 3 && ok; ++d) ok = p->L[d] > 0 && p->Ng[d] >= p->P && p->Ng[d] >= 4;
-    if (!ok) { g_create_err = "invalid pce_params (need xi,rc,a,eps_f>0; P even in 4..32; Ng>=P; max_iter>0)"; return PCE_EINVAL; }
+    if (ok && p->P_matvec != 0) ok = p->P_matvec >= 4 && p->P_matvec <= p->P && p->P_matvec % 2 == 0;
+    if (!ok) { g_create_err = "invalid pce_params (need xi,rc,a,eps_f>0; P even in 4..32; P_matvec 0 or even in 4..P; Ng>=P; max_iter>0)"; return PCE_EINVAL; }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         g_create_err = "no CUDA device: this library has no CPU fallback";
@@ -257,6 +279,13 @@ static int positions_impl(pce_ctx* c, const double* x, const double* y, const do
             if ((rc = wave_window_coef(c, c->wall))) return rc;
             if ((rc = wave_window_coef(c, c->wbead))) return rc;
         }
+        if (c->wmv == &c->wbead_s) {  // the beads once more for the narrower window of the solver matvec
+            wave_select(c, 1);
+            rc = bins_build(c, c->wbead_s, c->x, c->y, c->z);
+            if (!rc) rc = c->use_cols ? wave_cols_build(c, c->wbead_s) : wave_window_coef(c, c->wbead_s);
+            wave_select(c, 0);
+            if (rc) return rc;
+        }
         if ((rc = bodies_setup(c))) return rc;
     }
     if ((rc = real_csr_build(c, c->bead))) return rc;
@@ -308,6 +337,15 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     } else {
         if ((rc = wave_coef_alloc(c, c->wall))) return rc;
         if ((rc = wave_coef_alloc(c, c->wbead))) return rc;
+    }
+    c->wmv = &c->wbead;
+    if (c->P_mv != c->p.P && c->Nbead > 0) {
+        wave_select(c, 1);
+        rc = bins_alloc_tiles(c, c->wbead_s, c->Nbead, 8);
+        if (!rc) rc = c->use_cols ? wave_cols_alloc(c, c->wbead_s) : wave_coef_alloc(c, c->wbead_s);
+        wave_select(c, 0);
+        if (rc) return rc;
+        c->wmv = &c->wbead_s;
     }
     PCE_CUDA(c, cudaMalloc(&c->csr_ptr, ((size_t)c->Nbead + 2) * sizeof(int)));
     ALLOC_D(c->w_real, N); ALLOC_D(c->w_wave, N); ALLOC_D(c->w_ex, N); ALLOC_D(c->w_ey, N); ALLOC_D(c->w_ez, N);
@@ -454,11 +492,14 @@ int op_matvec_bead_sorted(pce_ctx* c)
     c->tm.n_matvec_bead++;
     c->tm.n_fft_pairs++;
     c->in_bead_matvec = true;
+    wave_select(c, 1);  // the solver's window (P_matvec points)
+    Bins& wb = *c->wmv;
     int rc = real_csr_spmv(c, c->bead, c->w_real);
-    if (!rc) rc = c->use_cols ? wave_spread_cols(c, c->wbead) : wave_spread_bricks(c, c->wbead);
+    if (!rc) rc = c->use_cols ? wave_spread_cols(c, wb) : wave_spread_bricks(c, wb);
     if (!rc) rc = wave_fft_scale_ifft(c);
-    if (!rc) rc = c->use_cols ? wave_gather_cols(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr)
-                              : wave_gather_bricks(c, c->wbead, false, c->w_wave, nullptr, nullptr, nullptr);
+    if (!rc) rc = c->use_cols ? wave_gather_cols(c, wb, false, c->w_wave, nullptr, nullptr, nullptr)
+                              : wave_gather_bricks(c, wb, false, c->w_wave, nullptr, nullptr, nullptr);
+    wave_select(c, 0);
     c->in_bead_matvec = false;
     return rc;
 }
@@ -468,7 +509,9 @@ int op_matvec_bead(pce_ctx* c, const double* q, double* psi)
     c->tm.n_matvec_bead++;
     c->tm.n_fft_pairs++;
     c->in_bead_matvec = true;
-    int rc = apply_operator(c, c->bead, c->wbead, c->bead, c->wbead, true, q, psi, nullptr, nullptr, nullptr);
+    wave_select(c, 1);
+    int rc = apply_operator(c, c->bead, *c->wmv, c->bead, *c->wmv, true, q, psi, nullptr, nullptr, nullptr);
+    wave_select(c, 0);
     c->in_bead_matvec = false;
     return rc;
 }
@@ -641,6 +684,7 @@ extern "C" int pce_get_info(const pce_ctx* c, pce_info* info)
     info->bytes_workspace = c->bytes;
     info->bytes_precond = c->pc_bytes;
     info->n_precond_blocks = c->pc_on ? c->pc_nblock : 0;
+    info->P_matvec = c->P_mv;
     info->fft_mode = c->use_fftxy ? 2 : c->use_zfft ? 1 : 0;
     return PCE_OK;
 }

@@ -121,7 +121,9 @@ struct pce_ctx {
     RealConst rk;
     RealTable rt;              // real-space kernel table (device pointer), realtab.h
     double* rt_dev = nullptr;
-    WaveConst wk;
+    WaveConst wk;              // the ACTIVE wave-space constants (wave_select): a copy of wset[0] or wset[1]
+    WaveConst wset[2];         // [0]: window of P points (evaluations, right-hand side); [1]: P_matvec points (solver matvec)
+    int P_mv = 0;              // = P_matvec (or P)
     double V = 0, eta[3], h[3];
     double kconst = 0;  // 1/(4 xi^2 V eps)
 
@@ -136,7 +138,9 @@ struct pce_ctx {
     double *X = nullptr, *Y = nullptr, *Z = nullptr;     // [Nbody] centres (unwrapped about first bead)
 
     Bins all, bead;    // real-space linked cells (all particles / conductor beads)
-    Bins wall, wbead;  // mesh tiles (spread / gather)
+    Bins wall, wbead;  // mesh tiles (spread / gather), window of P points
+    Bins wbead_s;      // the beads binned for the window of P_matvec points (only if P_matvec != P)
+    Bins* wmv = nullptr;  // the bead binning of the solver matvec: &wbead_s or &wbead
     int* scan_tmp = nullptr;  // block sums for the scans
     size_t scan_tmp_n = 0;
 
@@ -155,7 +159,8 @@ struct pce_ctx {
     bool have_plans = false;
     bool use_zfft = false;     // 2-D cuFFT per plane + fused z FFT / Green's function / inverse z FFT (zfft.cu)
     double2* ztw = nullptr;    // twiddles exp(-2 pi i m / N_z)
-    double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function
+    double* zexp = nullptr;    // per-axis Gaussian factors of the Green's function (active set)
+    double* zexp_set[2] = {nullptr, nullptr};
     double* zshape = nullptr;  // piecewise-polynomial table of the shape factor j0(ka)^2 / k^2 as a function of k^2
     int zshape_key_lo = 0, zshape_n = 0;
     bool use_fftxy = false;    // own (x, y) transforms, one HBM trip per plane and direction (fftxy.cu) instead of cuFFT 2-D plans
@@ -280,6 +285,9 @@ void realtab_build_host(double a, double xi, double rc, std::vector<double>& tab
 int realtab_upload(pce_ctx* c);
 void chebtab_build(double s_lo, double s_hi, long double (*f)(long double, const void*), const void* ctx, std::vector<double>& tab,
                    int& key_lo, int& n_int);
+
+// pce_api.cu
+void wave_select(pce_ctx* c, int which);  // 0: window of P points, 1: window of P_matvec points (solver matvec)
 
 // wave.cu
 int wave_fft_scale_ifft(pce_ctx* c);

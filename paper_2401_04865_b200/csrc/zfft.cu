@@ -182,16 +182,20 @@ int zfft_init(pce_ctx* c)
     stage_twiddles(n, tw);
     PCE_CUDA(c, cudaMalloc(&c->ztw, tw.size() * sizeof(double2)));
     PCE_CUDA(c, cudaMemcpy(c->ztw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice));
-    // per-axis factors exp(-(1 - eta_d) k_d^2 / 4 xi^2) of eq. 26: [kx = 0..Nx/2 | ky = 0..Ny/2 | kz = 0..Nz/2]
+    // per-axis factors exp(-(1 - eta_d) k_d^2 / 4 xi^2) of eq. 26: [kx = 0..Nx/2 | ky = 0..Ny/2 | kz = 0..Nz/2], one set per window
+    // (eta depends on P, eq. 31)
     const int cnt[3] = {c->wk.Nxh, c->p.Ng[1] / 2 + 1, n / 2 + 1};
-    std::vector<double> ze;
-    for (int d = 0; d < 3; ++d)
-        for (int i = 0; i < cnt[d]; ++i) {
-            const double k = c->wk.kfac[d] * i;
-            ze.push_back(std::exp(-c->wk.gexp[d] * k * k));
-        }
-    PCE_CUDA(c, cudaMalloc(&c->zexp, ze.size() * sizeof(double)));
-    PCE_CUDA(c, cudaMemcpy(c->zexp, ze.data(), ze.size() * sizeof(double), cudaMemcpyHostToDevice));
+    for (int s = 0; s < 2; ++s) {
+        std::vector<double> ze;
+        for (int d = 0; d < 3; ++d)
+            for (int i = 0; i < cnt[d]; ++i) {
+                const double k = c->wset[s].kfac[d] * i;
+                ze.push_back(std::exp(-c->wset[s].gexp[d] * k * k));
+            }
+        PCE_CUDA(c, cudaMalloc(&c->zexp_set[s], ze.size() * sizeof(double)));
+        PCE_CUDA(c, cudaMemcpy(c->zexp_set[s], ze.data(), ze.size() * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    c->zexp = c->zexp_set[0];
     // shape factor j0(ka)^2 / k^2 (eq. 9 / eq. 26) as a function of s = k^2 between the smallest and the largest mesh wavenumber
     double smin = 1e300, smax = 0.0;
     for (int d = 0; d < 3; ++d) {

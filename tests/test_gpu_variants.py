@@ -225,3 +225,32 @@ def test_large_mesh_passes_against_the_oracle_on_full_vectors(ng):
     assert rel(f["f"].cpu().numpy(), oo["f"]) < 1e-8
     assert body_vector_error(f["T"].cpu().numpy(), oo["T"], oo["f"])[0] < 1e-8
     ctx.close()
+
+
+def test_narrower_window_for_the_solver_matvec():
+    """pce_params.P_matvec = P - 2: the solver's bead-only matvec spreads and gathers with 18 instead of 20 support points (its own
+    bead binning, hit lists and Green's-function tables).  Potentials, and with them the induced charges, stay within the 1e-9
+    bar; the final evaluation (fields, forces) still uses P."""
+    import torch
+    import paper_2401_04865_b200 as pce
+    pce.build()
+    w = wl.config2(d=3.0)
+    rng = np.random.default_rng(4)
+    qb = rng.normal(size=w.N_bead)
+    psi_o = orc.ewald_eval(w.x[:w.N_bead], qb, w.L, w.a, field=False)
+    qo, Phio, _ = orc.solve_induced(w.x, w.body_offset, w.Q_body, w.q_ion, w.E0, w.L, w.a)
+    oo = orc.forces_torques(w.x, w.body_offset, qo, w.E0, w.L, w.a, Phi_body=Phio)
+    for fused in (True, False):
+        ctx = pce.context_for(w, P_matvec=18, fused_z=fused)
+        assert ctx.info()["P_matvec"] == 18 and ctx.params.P == 20
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        assert rel(ctx.matvec(torch.from_numpy(qb).cuda()).cpu().numpy(), psi_o) < 1e-9
+        q, Phi, info = ctx.solve(Q, qi, w.E0)
+        f = ctx.forces(q, w.E0)
+        assert info["converged"] and rel(q.cpu().numpy(), qo) < 1e-9
+        assert rel(f["psi"].cpu().numpy(), oo["psi"]) < 1e-9 and rel(f["f"].cpu().numpy(), oo["f"]) < 1e-8
+        assert rel(f["S"].cpu().numpy(), oo["S"]) < 1e-9
+        ctx.close()
+    with pytest.raises(pce.PceError):
+        pce.context_for(w, P_matvec=22)   # wider than P: refused
