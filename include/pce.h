@@ -257,6 +257,31 @@ int pce_bd_step(pce_ctx* ctx, const pce_bd_params* bp, const double* fx, const d
 int pce_radial_profile(pce_ctx* ctx, int body, const double* q, double r_lo, int n_bins,
                        double* counts, double* g, double* rho, double* Qcum);
 
+/* The same observables for a caller that must not allocate device memory -- an analysis hook inside a simulation engine
+ * whose own pool has claimed the GPU's memory (so a cudaMalloc may fail in the middle of a run), or one that runs between the
+ * engine's kernels, where cudaMalloc / cudaFree would stall the whole device.  No pce_ctx is needed and the call makes no
+ * cudaMalloc, cudaFree or allocating library call: its one scratch buffer, the integer shell counters, is a fixed
+ * 128 KiB array inside the library image (held by every GPU that loads libpce.so until the process exits).
+ *   stream  : cudaStream_t the work is enqueued on (NULL: default stream); the call does not wait for it
+ *   x, y, z, q_ion : device [n_ion], positions (anywhere; minimum image is taken) and charges of the IONS only
+ *   q_bead  : device [n_bead], charges of the beads of the body the profile is taken about (Q of eq. 48 is their sum;
+ *             n_bead = 0: Q = 0)
+ *   centre, L : host [3], the body's reference point X_i and the box edges;  a: particle radius, dr = 0.1 a
+ *   counts, g, rho, Qcum : device, as in pce_radial_profile, owned by the caller; any may be NULL, Qcum needs rho
+ *   err     : host buffer of err_len bytes (may be NULL) that receives the text of a failure
+ * Limit: n_bins <= PCE_PROFILE_STATIC_MAX_BINS; more is refused with PCE_EINVAL (split [r_lo, r_hi) over several calls --
+ * counts, g and rho of a shell do not depend on the other shells; only Qcum carries the running sum).
+ * Set-up: the first call made with a given device current looks up the device address of the counter array
+ * (cudaGetSymbolAddress, once per device, under a lock); make that first call before any stream capture is begun.
+ * Sharing: every call on a device uses the same counters.  Each call zeroes the part it uses on `stream` before binning, so
+ * calls enqueued one after another on one stream are independent; two calls that can overlap on the GPU (different streams,
+ * different host threads without ordering between them) race on the counters and both results are garbage. */
+#define PCE_PROFILE_STATIC_MAX_BINS 16384
+int pce_radial_profile_static(void* stream, int n_ion, const double* x, const double* y, const double* z, const double* q_ion,
+                              int n_bead, const double* q_bead, const double centre[3], const double L[3], double a,
+                              double r_lo, int n_bins, double* counts, double* g, double* rho, double* Qcum,
+                              char* err, int err_len);
+
 /* One whole pass of the hot path from HOST buffers (what bench.py's "e2e"
  * times): copy positions and charges to the device, rebuild cells, solve
  * eq. 13, evaluate forces, copy results back.  All pointers host; x,y,z [N];

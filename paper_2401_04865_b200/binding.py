@@ -23,6 +23,7 @@ EXPORTS = (
     "pce_matvec", "pce_evaluate", "pce_solve", "pce_forces", "pce_step_host", "pce_set_timing", "pce_get_timings",
     "pce_get_info", "pce_launch_count", "pce_real_kernel_host", "pce_measure_fp64_peaks", "pce_debug_poison_shared_memory",
     "pce_capacitance_columns", "pce_effective_permittivity", "pce_bd_step", "pce_radial_profile", "pce_set_centres",
+    "pce_radial_profile_static",
 )
 
 
@@ -100,6 +101,8 @@ def load():
     lib.pce_effective_permittivity.argtypes = [vp, dp, C.POINTER(PceSolveInfo)]
     lib.pce_bd_step.argtypes = [vp, C.POINTER(PceBdParams)] + [vp] * 7
     lib.pce_radial_profile.argtypes = [vp, C.c_int, vp, C.c_double, C.c_int] + [vp] * 4
+    lib.pce_radial_profile_static.argtypes = [vp, C.c_int, vp, vp, vp, vp, C.c_int, vp, dp, dp, C.c_double, C.c_double, C.c_int] + [vp] * 4 + \
+                                             [C.c_char_p, C.c_int]
     lib.pce_real_kernel_host.argtypes = [C.c_double] * 4 + [C.c_int, dp, dp, dp]
     for n in EXPORTS:
         if n not in ("pce_last_error", "pce_launch_count"):
@@ -155,6 +158,37 @@ def suggest_params(L, Ng, a, tol=1e-10, P=0) -> PceParams:
 
 def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+PROFILE_STATIC_MAX_BINS = 16384  # PCE_PROFILE_STATIC_MAX_BINS of include/pce.h
+
+
+def radial_profile_static(x, y, z, q_ion, q_bead, centre, L, a, r_lo, n_bins, out=None):
+    """pce_radial_profile_static: the observables of Context.radial_profile without a context and without any device-memory
+    allocation inside the library (its shell counters live in a fixed array of the library image) -- for callers that may not
+    cudaMalloc, e.g. an analysis hook inside a simulation engine that has handed all device memory to its own pool.
+    x, y, z, q_ion: contiguous CUDA float64 tensors of the ions; q_bead: charges of the body's beads (or None);
+    ``out``: dict of preallocated tensors counts[2 n], g[2 n], rho[n], Qcum[n] to write into (this wrapper makes them with
+    torch if not given: that allocation is the caller's, through torch's pool, not the library's).  n_bins is limited to
+    PROFILE_STATIC_MAX_BINS.  Work is enqueued on the current torch stream; calls that overlap on the GPU race on the shared
+    counters."""
+    import torch
+    n = int(x.numel())
+    for t in (x, y, z, q_ion):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n, "need contiguous cuda f64"
+    nb = 0 if q_bead is None else int(q_bead.numel())
+    if q_bead is not None:
+        assert q_bead.is_cuda and q_bead.dtype == torch.float64 and q_bead.is_contiguous(), "need contiguous cuda f64"
+    if out is None:
+        m = max(int(n_bins), 0)
+        out = {k: torch.empty(s, dtype=torch.float64, device=x.device) for k, s in (("counts", 2 * m), ("g", 2 * m), ("rho", m), ("Qcum", m))}
+    err = C.create_string_buffer(512)
+    rc = load().pce_radial_profile_static(C.c_void_p(torch.cuda.current_stream().cuda_stream), n, _ptr(x), _ptr(y), _ptr(z), _ptr(q_ion), nb,
+                                          _ptr(q_bead), _d3(centre), _d3(L), float(a), float(r_lo), int(n_bins), _ptr(out.get("counts")),
+                                          _ptr(out.get("g")), _ptr(out.get("rho")), _ptr(out.get("Qcum")), err, len(err))
+    if rc:
+        raise PceError(rc, err.value.decode())
+    return out
 
 
 class Context:
