@@ -97,6 +97,8 @@ typedef struct {
     double rel_resid;   /* final |P(b - M q)| / (|P r.E0|^2 + |P psi0|^2)^(1/2), psi0 = potential of the uniform starting
                            charges and the ions; a warm-started solve keeps the scale of the last cold solve if larger */
     int    converged;   /* 1 if rel_resid <= tol_solver */
+    int    graph_replays; /* iterations enqueued as replays of the captured CUDA graph (0: plain kernel launches -- timing
+                           enabled, PCE_NO_GRAPH=1, or a context on the legacy default stream, which cannot be captured) */
 } pce_solve_info;
 
 /* Per-pass device times (ms, CUDA events on the context's stream) summed over

@@ -34,7 +34,8 @@ class PceParams(C.Structure):
 
 
 class PceSolveInfo(C.Structure):
-    _fields_ = [("iters", C.c_int), ("matvecs", C.c_int), ("rel_resid", C.c_double), ("converged", C.c_int)]
+    _fields_ = [("iters", C.c_int), ("matvecs", C.c_int), ("rel_resid", C.c_double), ("converged", C.c_int),
+                ("graph_replays", C.c_int)]
 
 
 class PceBdParams(C.Structure):
@@ -281,7 +282,8 @@ class Context:
         info = PceSolveInfo()
         self._ck(self.lib.pce_solve(self.h, _ptr(Q_body), _ptr(q_ion) if self.N - self.N_bead else None, _d3(E0), warm,
                                     _ptr(q), _ptr(Phi), C.byref(info)), allow=(PCE_ENOCONV,) if allow_noconv else ())
-        return q, Phi, {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid, "converged": bool(info.converged)}
+        return q, Phi, {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid, "converged": bool(info.converged),
+                        "graph_replays": info.graph_replays}
 
     def forces(self, q, E0):
         self._chk(q, self.N)
@@ -345,7 +347,8 @@ class Context:
                                              hp(out.get("Phi")), hp(out.get("fx")), hp(out.get("fy")), hp(out.get("fz")),
                                              hp(out.get("F")), hp(out.get("T")), hp(out.get("S")), hp(out.get("U")),
                                              C.byref(info)), allow=(PCE_ENOCONV,))
-        return {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid, "converged": bool(info.converged), "rc": rc}
+        return {"iters": info.iters, "matvecs": info.matvecs, "rel_resid": info.rel_resid, "converged": bool(info.converged), "rc": rc,
+                "graph_replays": info.graph_replays}
 
     # ---- reports
     def set_timing(self, on=True):

@@ -193,6 +193,13 @@ k_resid_init(int nb, const int* __restrict__ off, const double* __restrict__ rx,
     }
 }
 
+// save (restore = 0) / put back (restore = 1) the residual scale of the last cold-start solve around internal solves
+__global__ void k_ref_cold_keep(CgState* __restrict__ st, int restore)
+{
+    if (restore) st->ref_cold = st->ref_saved;
+    else st->ref_saved = st->ref_cold;
+}
+
 // plain system M q = b from q = 0: g = b; ref = |b|
 __global__ void __launch_bounds__(BT)
 k_resid_init_plain(int n, const double* __restrict__ b, double* __restrict__ g, double* __restrict__ q, double* __restrict__ psi,
@@ -378,14 +385,20 @@ static int krylov_alloc(pce_ctx* c)
     return PCE_OK;
 }
 
-void krylov_invalidate_graph(pce_ctx* c)
+// The captured iteration bakes in device pointers (csr_col / csr_val, gather_part, the hit and pair lists), sizes (nnz, n_items,
+// n_pairs) and grid dimensions, all of which change with the positions or with a reallocation: whoever changes one of them calls
+// this, and the next solve captures the iteration again (updating the instantiated graph in place where the topology is unchanged).
+void krylov_invalidate_graph(pce_ctx* c) { c->cg_graph_stale = true; }
+
+static void destroy_graph(pce_ctx* c)
 {
     if (c->cg_graph) { cudaGraphExecDestroy(c->cg_graph); c->cg_graph = nullptr; }
+    c->cg_graph_stale = false;
 }
 
 void krylov_free(pce_ctx* c)
 {
-    krylov_invalidate_graph(c);
+    destroy_graph(c);
     cudaFree(c->cg_state);
     if (c->cg_host) cudaFreeHost(c->cg_host);
     c->cg_state = nullptr; c->cg_host = nullptr; c->cg_host_dev = nullptr; c->cg_graph_failed = false;
@@ -438,12 +451,14 @@ static bool graphs_enabled()
     return on == 1;
 }
 
-// capture one iteration into a graph (once per system; arrays it touches are owned by the context)
+// capture one iteration into a graph (again after every krylov_invalidate_graph; arrays it touches are owned by the context).
+// The legacy default stream cannot be captured (cudaStreamBeginCapture fails on it): a context created on it runs plain launches.
 static int capture_iteration(pce_ctx* c)
 {
     cudaGraph_t g = nullptr;
     const long long l0 = c->launches;
-    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->cg_graph_failed = true; return PCE_OK; }
+    c->cg_graph_stale = false;
+    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); destroy_graph(c); c->cg_graph_failed = true; return PCE_OK; }
     const int rc = enqueue_iteration(c);
     const cudaError_t e = cudaStreamEndCapture(c->st, &g);
     c->cg_graph_launches = c->launches - l0;
@@ -451,10 +466,15 @@ static int capture_iteration(pce_ctx* c)
     if (rc != PCE_OK || e != cudaSuccess || !g) {
         cudaGetLastError();
         if (g) cudaGraphDestroy(g);
+        destroy_graph(c);
         c->cg_graph_failed = true;  // fall back to plain launches
         return PCE_OK;
     }
-    if (cudaGraphInstantiate(&c->cg_graph, g, 0) != cudaSuccess) { cudaGetLastError(); c->cg_graph = nullptr; c->cg_graph_failed = true; }
+    if (c->cg_graph) {  // same topology, new arguments: update in place; otherwise instantiate afresh
+        cudaGraphExecUpdateResultInfo upd;
+        if (cudaGraphExecUpdate(c->cg_graph, g, &upd) != cudaSuccess) { cudaGetLastError(); destroy_graph(c); }
+    }
+    if (!c->cg_graph && cudaGraphInstantiate(&c->cg_graph, g, 0) != cudaSuccess) { cudaGetLastError(); c->cg_graph = nullptr; c->cg_graph_failed = true; }
     cudaGraphDestroy(g);
     return PCE_OK;
 }
@@ -484,7 +504,7 @@ static int run_iterations(pce_ctx* c, pce_solve_info* inf)
     const int maxit = c->p.max_iter;
     int rc = PCE_OK;
     const bool use_graph = !c->timing && graphs_enabled() && !c->cg_graph_failed;
-    if (use_graph && !c->cg_graph) {
+    if (use_graph && (!c->cg_graph || c->cg_graph_stale)) {
         if ((rc = capture_iteration(c))) return rc;
     }
     // iterations kept in flight: large meshes take milliseconds per iteration (an unneeded replay costs its cuFFT passes), small
@@ -498,6 +518,7 @@ static int run_iterations(pce_ctx* c, pce_solve_info* inf)
         if (use_graph && c->cg_graph) {
             PCE_CUDA(c, cudaGraphLaunch(c->cg_graph, c->st));
             c->launches += c->cg_graph_launches;
+            inf->graph_replays++;
         } else if ((rc = enqueue_iteration(c))) return rc;
         ++launched;
     }
@@ -751,6 +772,7 @@ int capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_so
         c->launches++;
         worst.iters = worst.iters > inf.iters ? worst.iters : inf.iters;
         worst.matvecs += inf.matvecs;
+        worst.graph_replays += inf.graph_replays;
         worst.rel_resid = worst.rel_resid > inf.rel_resid ? worst.rel_resid : inf.rel_resid;
         worst.converged = worst.converged && inf.converged;
     }
@@ -767,7 +789,17 @@ int effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info)
     const int nb = c->Nbody, N = c->N;
     pce_solve_info worst = {0, 0, 0.0, 1};
     int rc_all = PCE_OK;
+    // ev_psi holds max(N, 4 N_body) doubles (pce_set_system): room for the 4 N_body moments of k_cap_moments
     double *zeros = c->ev_ey, *q = c->ev_ez, *Phi = c->ev_ex, *mom = c->ev_psi;
+    // the three unit-field solves below are cold starts of a problem of their own scale: keep the residual scale of the caller's
+    // last cold pce_solve, which its next warm-started solve measures its tolerance against
+    int rc0 = krylov_alloc(c);
+    if (rc0) return rc0;
+    struct RefColdKeeper {
+        pce_ctx* c;
+        explicit RefColdKeeper(pce_ctx* c_) : c(c_) { k_ref_cold_keep<<<1, 1, 0, c->st>>>(c->cg_state, 0); c->launches++; }
+        ~RefColdKeeper() { k_ref_cold_keep<<<1, 1, 0, c->st>>>(c->cg_state, 1); c->launches++; }
+    } keep(c);
     PCE_CUDA(c, cudaMemsetAsync(zeros, 0, (size_t)N * sizeof(double), c->st));
     std::vector<double> h((size_t)4 * nb);
     for (int d = 0; d < 3; ++d) {
@@ -787,6 +819,7 @@ int effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info)
         }
         worst.iters = worst.iters > inf.iters ? worst.iters : inf.iters;
         worst.matvecs += inf.matvecs;
+        worst.graph_replays += inf.graph_replays;
         worst.rel_resid = worst.rel_resid > inf.rel_resid ? worst.rel_resid : inf.rel_resid;
         worst.converged = worst.converged && inf.converged;
     }

@@ -36,14 +36,14 @@ extern "C" int pce_suggest_params(const double L[3], const int Ng[3], double a, 
 }
 
 // ---------------------------------------------------------------- timing
-static void timing_begin(pce_ctx* c)
+void timing_begin(pce_ctx* c)
 {
     std::memset(&c->tm, 0, sizeof(c->tm));
     c->recs.clear();
     c->ev_used = 0;
 }
 
-static void timing_end(pce_ctx* c)
+void timing_end(pce_ctx* c)
 {
     if (!c->timing) return;
     cudaStreamSynchronize(c->st);
@@ -265,6 +265,7 @@ static void cell_layout(const pce_params& p, int nc[3], int range[3])
 static int positions_impl(pce_ctx* c, const double* x, const double* y, const double* z)
 {
     int rc;
+    krylov_invalidate_graph(c);  // list sizes, grid dimensions and possibly reallocated buffers are baked into the captured iteration
     {
         PassTimer t(c, PASS_CELLS);
         if ((rc = wrap_positions(c, c->N, x, y, z, c->x, c->y, c->z))) return rc;
@@ -352,7 +353,8 @@ extern "C" int pce_set_system(pce_ctx* c, int N, int N_body, const int* body_off
     ALLOC_D(c->w_kx, N); ALLOC_D(c->w_ky, N); ALLOC_D(c->w_kz, N);
     ALLOC_D(c->cg_g, c->Nbead); ALLOC_D(c->cg_p, c->Nbead); ALLOC_D(c->cg_t, c->Nbead); ALLOC_D(c->cg_ap, c->Nbead);
     ALLOC_D(c->cg_psi, c->Nbead); ALLOC_D(c->cg_q, c->Nbead);
-    ALLOC_D(c->ev_psi, N); ALLOC_D(c->ev_ex, N); ALLOC_D(c->ev_ey, N); ALLOC_D(c->ev_ez, N);
+    ALLOC_D(c->ev_psi, N > 4 * N_body ? N : 4 * N_body);  // also the 4 N_body body moments of pce_effective_permittivity
+    ALLOC_D(c->ev_ex, N); ALLOC_D(c->ev_ey, N); ALLOC_D(c->ev_ez, N);
     ALLOC_D(c->cg_part, 3 * (N_body > 1024 ? N_body : 1024));
     ALLOC_D(c->cg_z, c->Nbead); ALLOC_D(c->pc_mean, N_body);
     c->have_system = true;

@@ -103,6 +103,7 @@ struct CgState {
     double pap, gg;      // p.Ap, |g|^2
     double psum;         // sum of the search direction (k = 0 constant of the operator, reading A1)
     double ref, ref_cold;  // residual scale; the one of the last cold-start solve
+    double ref_saved;      // ref_cold of the caller's solves while pce_effective_permittivity runs its own
     double tol;
     int it, maxit, done, project;  // project = 1: eq. 13 on the per-body-mean-projected subspace; 0: plain M q = b
     unsigned cnt[8];     // arrival counters of the last-block-done reductions
@@ -192,6 +193,7 @@ struct pce_ctx {
     CgHostStatus* cg_host_dev = nullptr;  // its device address
     cudaGraphExec_t cg_graph = nullptr; // one captured Krylov iteration (matvec + vector kernels)
     bool cg_graph_failed = false;
+    bool cg_graph_stale = false;        // positions / a buffer the graph names changed: capture again before the next replay
     long long cg_graph_launches = 0;    // kernels of this library inside one replay
     const int* skip_flag = nullptr;     // when set, the operator kernels return at once if *skip_flag != 0 (solver converged)
     // block-Jacobi preconditioner (precond.cu)
@@ -330,6 +332,14 @@ int capacitance_columns(pce_ctx* c, int ncol, const int* cols, double* C, pce_so
 int effective_permittivity(pce_ctx* c, double eps_eff[9], pce_solve_info* info);
 void krylov_free(pce_ctx* c);
 void krylov_invalidate_graph(pce_ctx* c);
+// per-call timing records (pce_api.cu): every entry point that opens PassTimers brackets itself with these
+void timing_begin(pce_ctx* c);
+void timing_end(pce_ctx* c);
+struct TimingScope {
+    pce_ctx* c;
+    explicit TimingScope(pce_ctx* c_) : c(c_) { timing_begin(c); }
+    ~TimingScope() { timing_end(c); }
+};
 int op_matvec_bead_sorted(pce_ctx* c);  // sorted charges in bead.qs / wbead.qs -> w_real / w_wave (sorted orders)
 int forces_all(pce_ctx* c, const double* q, const double E0[3], double* fx, double* fy, double* fz, double* F, double* T,
                double* S, double* U_body, double* U_tot, double* psi_out);

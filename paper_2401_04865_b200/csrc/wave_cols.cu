@@ -852,6 +852,7 @@ int wave_gather_cols(pce_ctx* c, const Bins& b, bool field, double* psi_s, doubl
     if (det) {  // partial sums per (brick, hit) pair and quantity
         const long long need = (long long)b.n_pairs * nq;
         if (need > c->part_cap) {
+            krylov_invalidate_graph(c);  // the captured iteration names the old buffer
             cudaFree(c->gather_part);
             c->gather_part = nullptr;
             c->bytes -= c->part_cap * 8;
