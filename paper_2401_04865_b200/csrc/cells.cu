@@ -116,7 +116,7 @@ __global__ void k_gather_perm(int n, const int* __restrict__ perm, const double*
     if (i < n) out[(size_t)i * stride] = in[perm[i]];
 }
 
-// out[i * out_stride] = in[perm[i]] (stride 16: the charge slot of the 128-byte hit records, wave_cols.cu)
+// out[i * out_stride] = in[perm[i]] (stride HITREC_Q_STRIDE = 8: the charge slot of the 64-byte hit records, wave_cols.cu)
 int gather_by_perm(pce_ctx* c, int n, const int* perm, const double* in, double* out, int out_stride)
 {
     if (n == 0) return PCE_OK;

@@ -310,6 +310,7 @@ extern "C" int pce_bd_step(pce_ctx* c, const pce_bd_params* bp, const double* fx
     if (!(bp->dt > 0.0) || !(bp->gamma > 0.0) || !(bp->kT >= 0.0)) { c->err = "pce_bd_step: need dt > 0, gamma > 0, kT >= 0"; return PCE_EINVAL; }
     int rc = dynamics_alloc(c);
     if (rc) return rc;
+    TimingScope timed(c);  // the step's passes (hard spheres under "other", the rebuild under cells / real) in pce_get_timings
     const int N = c->N;
     {
         PassTimer t(c, PASS_OTHER);
@@ -346,6 +347,8 @@ extern "C" int pce_radial_profile(pce_ctx* c, int body, const double* q, double 
     if (!c->have_system) { c->err = "pce_radial_profile before pce_set_system"; return PCE_ESTATE; }
     if (!q || body < 0 || body >= c->Nbody || n_bins <= 0 || !(r_lo >= 0.0)) { c->err = "pce_radial_profile: bad arguments"; return PCE_EINVAL; }
     if (Qcum && !rho) { c->err = "pce_radial_profile: Qcum needs rho"; return PCE_EINVAL; }
+    TimingScope timed(c);
+    PassTimer t(c, PASS_OTHER);
     if (c->prof_cnt_n < 2 * n_bins) {
         cudaFree(c->prof_cnt);
         c->prof_cnt = nullptr; c->prof_cnt_n = 0;
