@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--fig3d", action="store_true",
                     help="the paper's timing workload (PAPER.md:325, Fig. 3d): induced-charge solve of FCC arrays vs total bead count; "
                          "prints its own JSON line and exits")
+    ap.add_argument("--no-configs", action="store_true", help="skip the short runs of BASELINE.json configs 1-4 reported in 'configs'")
     ap.add_argument("--bd", type=int, default=0, metavar="STEPS",
                     help="also run STEPS Brownian-dynamics steps on the device (solve + forces + pce_bd_step; config 3: 100, dt = 1e-4 a^2)")
     return ap.parse_args()
@@ -69,14 +70,33 @@ def make_workload(idx, rank=0):
     return wl.config5(seed=seed)
 
 
+def ewald_params(L, Ng, a, tol, P=0):
+    """(xi, r_c, P) from a tolerance by eqs. 28, 23 (+2a for shells, reading A14) and 32 -- the arithmetic the
+    header states for pce_suggest_params, restated here so that the reference arm can describe its configuration without loading
+    the product library (tests/test_abi.py holds the two to each other)."""
+    import math
+    L = np.broadcast_to(np.asarray(L, dtype=np.float64), (3,))
+    Ng = np.broadcast_to(np.asarray(Ng), (3,))
+    s = math.sqrt(-math.log(tol))
+    kc = min(math.pi * (int(n) - 1) / float(l) for n, l in zip(Ng, L))
+    xi = kc / (2.0 * s)
+    rc = s / xi + 2.0 * a
+    if P <= 0:
+        P = 2 * math.ceil(((2.0 / math.pi) * (-math.log(tol)) + 4.0) / 2.0)
+    P = min(max(P, 4), 32)
+    for n in Ng:
+        if P > int(n):
+            P = int(n) & ~1
+    return xi, rc, int(P)
+
+
 def config_dict(w, args):
-    """The `config` object of the JSON line: the workload and the Ewald parameters that follow from it (pure host arithmetic,
-    pce_suggest_params), identical in both arms so that the driver can pair them."""
-    import paper_2401_04865_b200 as pce
-    prm = pce.suggest_params(w.L, w.Ng, w.a, args.tol, args.P)
+    """The `config` object of the JSON line: the workload and the Ewald parameters that follow from it (pure host arithmetic),
+    identical in both arms so that the driver can pair them.  No import of the product package: the reference arm calls this."""
+    xi, rc, P = ewald_params(w.L, w.Ng, w.a, args.tol, args.P)
     grid_bytes = 8 * int(np.prod(w.Ng))
     return {"workload": w.name, "N": w.N, "N_bead": w.N_bead, "N_body": w.N_body, "grid": [int(g) for g in w.Ng],
-            "P": int(prm.P), "P_matvec": int(args.P_matvec or prm.P_matvec), "xi": prm.xi, "rc": prm.rc, "ewald_tol": args.tol, "solver_tol": args.tol_solver,
+            "P": P, "P_matvec": int(args.P_matvec or P), "xi": xi, "rc": rc, "ewald_tol": args.tol, "solver_tol": args.tol_solver,
             "l2": "flushed between timed steps" if grid_bytes < 256 << 20 else "inputs larger than L2 (grids %.2f GB)" % (grid_bytes * 3 / 1e9),
             "multi_gpu": "replicas only"}
 
@@ -219,6 +239,60 @@ def reduce_over_ranks(dist, ms, count, device):
     return float(t.item()), float(c.item())
 
 
+def m1_algorithmic_bytes(w, nnz_near):
+    """Algorithmic bytes of one bead-only matvec: spread, two transforms, scale, gather, cached near field."""
+    Ng3, Nk = int(np.prod(w.Ng)), int((w.Ng[0] // 2 + 1) * w.Ng[1] * w.Ng[2])
+    return (32 * w.N_bead + 8 * Ng3) + 2 * (8 * Ng3 + 16 * Nk) + 32 * Nk + (8 * Ng3 + 40 * w.N_bead) + 12 * nnz_near + 20 * w.N_bead
+
+
+def small_config_row(pce, torch, idx, args, hbm_peak, steps=10, warmup=3):
+    """One of BASELINE.json's smaller configurations through the same whole step (set_positions + solve + forces), on a stream
+    of its own so that the solver's CUDA graph replays; L2 flushed between timed steps (their meshes fit in it)."""
+    w = make_workload(idx)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, stream=st)
+        x, y, z, Q, qi = pce.upload(w)
+        ctx.set_system(w.body_offset, x, y, z)
+        info = ctx.info()
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+        ms, its, replays, conv, resid = [], [], 0, True, 0.0
+        for i in range(warmup + steps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            ctx.set_positions(x, y, z)
+            q, Phi, si = ctx.solve(Q, qi, w.E0, allow_noconv=True)
+            ctx.forces(q, w.E0)
+            b.record()
+            torch.cuda.synchronize()
+            if i >= warmup:
+                ms.append(a.elapsed_time(b)); its.append(si["iters"]); replays += si["graph_replays"]
+                conv = conv and bool(si["converged"]); resid = max(resid, si["rel_resid"])
+        row = {"config": idx, "workload": w.name, "N": w.N, "N_bead": w.N_bead, "grid": [int(g) for g in w.Ng], "fft_mode": info["fft_mode"],
+               "ms_per_step": float(np.mean(ms)), "cg_iters": float(np.mean(its)), "converged": conv, "rel_resid": resid,
+               "graph_replays_per_step": replays / steps, "steps": steps}
+        if w.N_bead:
+            qb = torch.randn(w.N_bead, dtype=torch.float64, device="cuda")
+            ctx.matvec(qb)
+            reps = 50
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            for _ in range(reps):
+                ctx.matvec(qb)
+            b.record()
+            torch.cuda.synchronize()
+            m1 = a.elapsed_time(b) / reps
+            nbytes = m1_algorithmic_bytes(w, info["nnz_near"])
+            row.update({"m1_ms": m1, "m1_per_s": 1e3 / m1, "m1_frac_of_hbm_ceiling": (nbytes / (m1 * 1e-3)) / (hbm_peak * 1e9),
+                        "m1_note": "back-to-back applications, mesh resident in L2 at these sizes"})
+            row["value"] = float(np.sum(its)) / (float(np.sum(ms)) * 1e-3)  # M1 applications per second of whole steps, as the headline
+        ctx.close()
+    torch.cuda.synchronize()
+    return row
+
+
 # ---------------------------------------------------------------- our arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -235,8 +309,13 @@ def run_ours(args, rank, world, local_rank):
         pce.build()
     if dist:
         dist.barrier()
+    # a stream of our own: the legacy default stream cannot be captured, and the solver replays its iteration as a CUDA graph
+    # (solve.graph_replays says whether it did); everything below -- torch copies, events, the library -- is enqueued on it
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
     w = make_workload(args.config, rank)
-    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, deterministic=args.deterministic, P_matvec=args.P_matvec)
+    ctx = pce.context_for(w, tol=args.tol, P=args.P, tol_solver=args.tol_solver, deterministic=args.deterministic, P_matvec=args.P_matvec,
+                          stream=stream)
     x, y, z, Q, qi = pce.upload(w)
     ctx.set_system(w.body_offset, x, y, z)
     info = ctx.info()
@@ -263,7 +342,7 @@ def run_ours(args, rank, world, local_rank):
         dist.barrier()
     # ---- timed region: K whole steps, per-pass event timing OFF (no instrumentation inside the headline number)
     l0 = ctx.launch_count()
-    ms_steps, iters, n_apply = [], [], 0
+    ms_steps, iters, n_apply, n_m1, n_graph, all_converged = [], [], 0, 0, 0, True
     for _ in range(args.steps):
         if l2_flush is not None:
             l2_flush.fill_(1)
@@ -276,6 +355,9 @@ def run_ours(args, rank, world, local_rank):
         ms_steps.append(e0.elapsed_time(e1))
         iters.append(sinfo["iters"])
         n_apply += sinfo["matvecs"] + 1  # solver matvecs + right-hand-side evaluation, + the force evaluation
+        n_m1 += sinfo["iters"]           # the bead-only solver matvecs alone: what the reference arm counts
+        n_graph += sinfo["graph_replays"]
+        all_converged = all_converged and bool(sinfo["converged"])
     launches = ctx.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     # ---- the same K steps again with the library's per-pass CUDA events on: per-kernel durations for the rooflines
@@ -294,8 +376,12 @@ def run_ours(args, rank, world, local_rank):
         ms_solve.append(tms[1]["total"])
     ctx.set_timing(False)
     total_ms = float(sum(ms_steps))
+    _, n_m1_all = reduce_over_ranks(dist, total_ms, n_m1, "cuda")
     total_ms, n_apply_all = reduce_over_ranks(dist, total_ms, n_apply, "cuda")
-    value = n_apply_all / (total_ms * 1e-3)
+    # headline: M1 applications (bead-only solver matvecs, the unit the reference arm times) per second of WHOLE steps -- the two
+    # full evaluations, the list rebuilds and the force pass of every step are in the denominator and count for nothing above it
+    value = n_m1_all / (total_ms * 1e-3)
+    value_all = n_apply_all / (total_ms * 1e-3)
 
     # ---- the two operator flavours on their own (CUDA events around back-to-back applications, this stream)
     def time_op(fn, reps):
@@ -362,13 +448,17 @@ def run_ours(args, rank, world, local_rank):
         n_e2e = 0
         for _ in range(args.steps):
             si = ctx.step_host(hx, hy, hz, hQ, hqi, w.E0, outb)
-            n_e2e += si["matvecs"] + 1
+            n_e2e += si["iters"]
         ev1.record()
         torch.cuda.synchronize()
         ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))  # the call is synchronous: host clock bounds it
         ms, n_e2e = reduce_over_ranks(dist, ms, n_e2e, "cuda")
         e2e = {"value": n_e2e / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * (3 * w.N + nb + w.N_ion),
                "d2h_bytes_per_step": 8 * (w.N + nb + 3 * w.N + 9 * nb + 3), "ms_per_step": ms / args.steps}
+    # ---- the other configurations of BASELINE.json, briefly (default run only: one GPU, config 5 as the headline)
+    cfg_rows = None
+    if world == 1 and args.config == 5 and not args.no_configs:
+        cfg_rows = [small_config_row(pce, torch, i, args, hbm_peak) for i in (1, 2, 3, 4)]
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -404,7 +494,7 @@ def run_ours(args, rank, world, local_rank):
                 2: "own (x, y) passes per mesh plane (fftxy.cu: one HBM trip per plane and direction); the 'scale' pass is the fused "
                    "z FFT + Green's function + inverse z FFT kernel; no library call on the path"}[info["fft_mode"]]
     # HBM ceiling of the bead-only matvec: the algorithmic bytes of all its passes at the measured copy rate
-    m1_bytes = (32 * w.N_bead + 8 * Ng3) + 2 * (8 * Ng3 + 16 * Nk) + 32 * Nk + (8 * Ng3 + 40 * w.N_bead) + 12 * info["nnz_near"] + 20 * w.N_bead
+    m1_bytes = m1_algorithmic_bytes(w, info["nnz_near"])
     if "m1_bead_matvec" in flavours:
         flavours["m1_bead_matvec"].update({"algorithmic_bytes": m1_bytes, "hbm_ceiling_per_s": hbm_peak * 1e9 / m1_bytes,
                                            "frac_of_hbm_ceiling": flavours["m1_bead_matvec"]["per_s"] * m1_bytes / (hbm_peak * 1e9)})
@@ -434,10 +524,13 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
+        "solve_converged": bool(all_converged), "solve_rel_resid": sinfo["rel_resid"], "solve_graph_replays_per_step": n_graph / args.steps,
+        "value_all_flavours": value_all,
         "config": config_dict(w, args),
         "run_info": {"cells": info["ncell"], "nnz_near": info["nnz_near"], "deterministic_gather": bool(args.deterministic),
                      "fft": fft_text},
-        "counts": "value = (M1 bead-only solver matvecs + M2 full evaluations) / whole-step time; the flavours are split in 'flavours'",
+        "counts": "value = M1 bead-only solver matvecs / whole-step time (same unit as the reference arm; e2e likewise); "
+                  "value_all_flavours adds the 2 full evaluations of every step to the numerator; the flavours are timed alone in 'flavours'",
         "flavours": flavours,
         "solve": {"cg_iters": iters, "solve_ms_per_step": float(np.mean(ms_solve)), "matvecs_bead": acc["n_matvec_bead"],
                   "evals_full": acc["n_eval_full"], "rel_resid": sinfo["rel_resid"], "converged": sinfo["converged"]},
@@ -448,6 +541,8 @@ def run_ours(args, rank, world, local_rank):
     }
     if bd:
         line["bd"] = bd
+    if cfg_rows:
+        line["configs"] = cfg_rows
     if not args.no_cpu_baseline:
         import oracle as orc
         orc.build()
